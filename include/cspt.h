@@ -1,0 +1,108 @@
+/* cspt.h -- C ABI of the B200-native CSPH-TVD time step.
+ *
+ * One explicit CSPH-TVD step (Khrapov, Khoperskov & Khoperskov 2019; PAPER.md
+ * section 2.2, Eq. (4)-(8)) on a uniform 3-D Cartesian grid for the ideal-gas
+ * Euler equations with an external potential psi (Eq. (1)-(3)):
+ * Lagrangian SPH-style predictor/corrector (Eq. (5)-(7)), Eulerian TVD stage
+ * (Eq. (8), (4)), CFL time step, boundary and gas-vacuum handling.  The readings
+ * of everything the paper leaves open are listed in DESIGN.md section 3.
+ *
+ * Conventions
+ *  - Every function returns an int status (CSPT_OK = 0, negative = error) unless
+ *    stated otherwise; nothing throws, aborts or prints.
+ *  - Arrays are dense, x fastest: element (i,j,k) at [ (k*ny + j)*nx + i ],
+ *    nx*ny*nz elements of the ctx's dtype (double for CSPT_F64, float for
+ *    CSPT_F32).  "device" pointers are CUDA device memory of the current
+ *    device, "host" pointers are ordinary (preferably pinned) host memory.
+ *  - Ownership: the caller owns every buffer it passes.  Inputs are copied,
+ *    outputs are written, the workspace is borrowed from cspt_create until
+ *    cspt_destroy.  The library owns only the small host-side ctx.
+ *  - All work is enqueued on the CUDA stream given to cspt_create; only the
+ *    functions marked "syncs" wait for it.
+ *  - There is no CPU fallback: without a CUDA device every call that needs one
+ *    returns CSPT_ECUDA.
+ */
+#ifndef CSPT_H
+#define CSPT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cspt_ctx cspt_ctx; /* opaque */
+
+enum { CSPT_F64 = 0, CSPT_F32 = 1 };
+/* boundary kind per face, order xlo,xhi,ylo,yhi,zlo,zhi (reading G16) */
+enum { CSPT_BC_PERIODIC = 0, CSPT_BC_OUTFLOW = 1, CSPT_BC_INFLOW = 2 };
+enum { CSPT_OK = 0, CSPT_EINVAL = -1, CSPT_ENOMEM = -2, CSPT_ECUDA = -3, CSPT_ESTATE = -4 };
+
+/* Bytes of device workspace cspt_create needs for this grid (0 if the arguments
+ * are invalid).  The caller allocates it (256-byte aligned), e.g. with torch. */
+size_t cspt_workspace_bytes(int nx, int ny, int nz, int dtype);
+
+/* Creates a solver for an nx*ny*nz grid of step h, adiabatic
+ * index gamma and the six boundary kinds.  workspace: device
+ * memory of at least cspt_workspace_bytes(); cuda_stream: a cudaStream_t
+ * (NULL = default stream).
+ * EINVAL: null out/bc/workspace, n < 1, n < 4 on a non-periodic axis, h <= 0,
+ * gamma <= 1, one face of an axis periodic and the other not, unknown dtype or
+ * boundary kind, workspace too small or misaligned.  In CSPT_F32 mode h, gamma,
+ * cfl and dt are rounded to float once at the API. */
+int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, const int bc[6],
+                int dtype, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Sets the state from primitives rho,u,v,w,p and the potential psi:
+ * U = (rho, rho u, E = p/(gamma-1) + rho |u|^2/2), f = -grad psi
+ * by the lattice SPH operator (reading G6), INFLOW faces capture their boundary
+ * layer (reading G16).  Device pointers; copied in; asynchronous. */
+int cspt_set_state(cspt_ctx*, const void* rho, const void* u, const void* v, const void* w,
+                   const void* p, const void* psi);
+/* Same, from HOST buffers (copied through the stream; syncs). */
+int cspt_set_state_host(cspt_ctx*, const void* rho, const void* u, const void* v, const void* w,
+                        const void* p, const void* psi);
+
+/* CFL time step (paper silent; reading G15): dt = cfl*h / max_cells(c + max(|u|,|v|,|w|)),
+ * c = sqrt(gamma p / rho), vacuum cells skipped; +inf if every cell is vacuum.
+ * Bit-exact and order independent (warp-shuffle + block max + integer atomic max
+ * of the IEEE bit pattern).  Writes *dt_host_out; syncs.  EINVAL: cfl <= 0. */
+int cspt_compute_dt(cspt_ctx*, double cfl, double* dt_host_out);
+
+/* One full step U^n -> U^{n+1} with time step dt (Eq. (4)-(8)): ghost fill,
+ * HFC/SUL predictor, HFC/SUL corrector, FGC, SUE.
+ * Asynchronous.  EINVAL: dt <= 0 or not finite.  ESTATE: no state set. */
+int cspt_step(cspt_ctx*, double dt);
+
+/* compute_dt followed by step with that dt, the time step staying on the
+ * device (no host sync).  dt_host_out may be NULL; if not, it is written and
+ * the call syncs.  A grid that is all vacuum (dt = +inf) is left unchanged. */
+int cspt_step_cfl(cspt_ctx*, double cfl, double* dt_host_out);
+
+/* Primitives rho,u,v,w,p of the current state (vacuum cells: u = v = w = p = 0).
+ * Device pointers; asynchronous. */
+int cspt_get_state(cspt_ctx*, void* rho, void* u, void* v, void* w, void* p);
+/* Conserved variables rho, rho u, rho v, rho w, E (parity is checked on these). */
+int cspt_get_conserved(cspt_ctx*, void* rho, void* mx, void* my, void* mz, void* E);
+/* Same, into HOST buffers (syncs). */
+int cspt_get_conserved_host(cspt_ctx*, void* rho, void* mx, void* my, void* mz, void* E);
+/* Overwrites the conserved variables, keeping psi/f and the captured inflow layers
+ * (checkpoint restore).  Device pointers. */
+int cspt_set_conserved(cspt_ctx*, const void* rho, const void* mx, const void* my, const void* mz,
+                       const void* E);
+/* mask[i] = 1 where rho <= rho_vac = 1e-12 (reading G9), else 0.  Device pointer. */
+int cspt_get_vacuum_mask(cspt_ctx*, unsigned char* mask);
+
+/* Number of kernel launches issued by this ctx so far (for bench.py's gpu_launches). */
+long long cspt_launch_count(const cspt_ctx*);
+/* Waits for the ctx's stream. */
+int cspt_sync(cspt_ctx*);
+/* Frees the ctx, never the workspace.  NULL is allowed. */
+void cspt_destroy(cspt_ctx*);
+/* Static string for a status code. */
+const char* cspt_strerror(int);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CSPT_H */

@@ -1,0 +1,182 @@
+"""Thin Python binding of the C ABI in include/cspt.h (same names, argument marshalling
+only).  PyTorch supplies device memory and streams; every step of the method runs in
+the CUDA kernels of libcspt.so.  There is no CPU fallback: if the library is missing
+or no CUDA device is present the calls fail loudly.
+"""
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcspt.so")
+
+F64, F32 = 0, 1
+BC_PERIODIC, BC_OUTFLOW, BC_INFLOW = 0, 1, 2
+OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
+
+# every symbol include/cspt.h declares: (name, restype, argtypes)
+_vp, _ci, _cd, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+_pd = ctypes.POINTER(ctypes.c_double)
+SYMBOLS = [
+    ("cspt_workspace_bytes", _sz, [_ci, _ci, _ci, _ci]),
+    ("cspt_create", _ci, [ctypes.POINTER(_vp), _ci, _ci, _ci, _cd, _cd, ctypes.POINTER(_ci), _ci, _vp, _sz, _vp]),
+    ("cspt_set_state", _ci, [_vp] * 7),
+    ("cspt_set_state_host", _ci, [_vp] * 7),
+    ("cspt_compute_dt", _ci, [_vp, _cd, _pd]),
+    ("cspt_step", _ci, [_vp, _cd]),
+    ("cspt_step_cfl", _ci, [_vp, _cd, _pd]),
+    ("cspt_get_state", _ci, [_vp] * 6),
+    ("cspt_get_conserved", _ci, [_vp] * 6),
+    ("cspt_get_conserved_host", _ci, [_vp] * 6),
+    ("cspt_set_conserved", _ci, [_vp] * 6),
+    ("cspt_get_vacuum_mask", _ci, [_vp, _vp]),
+    ("cspt_launch_count", ctypes.c_longlong, [_vp]),
+    ("cspt_sync", _ci, [_vp]),
+    ("cspt_destroy", None, [_vp]),
+    ("cspt_strerror", ctypes.c_char_p, [_ci]),
+]
+
+_lib = None
+
+
+class CsptError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        msg = lib().cspt_strerror(code).decode() if _lib is not None else str(code)
+        super().__init__("%s: %s (%d)" % (where, msg, code))
+
+
+def lib():
+    """Loads libcspt.so (built by `python -m paper_1912_04855_b200.build`); raises if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("libcspt.so is missing: run `python -m paper_1912_04855_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        for name, res, args in SYMBOLS:
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def _check(code, where):
+    if code != OK:
+        raise CsptError(code, where)
+
+
+def _dptr(t):
+    return ctypes.c_void_p(t.data_ptr())
+
+
+class Solver:
+    """One grid on the current CUDA device.  Tensors are (nz, ny, nx), x fastest."""
+
+    def __init__(self, nx, ny, nz, h, gamma, bc, dtype=F64, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("cspt needs a CUDA device (there is no CPU fallback)")
+        L = lib()
+        self.torch = torch
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.shape = (self.nz, self.ny, self.nx)
+        self.dtype = dtype
+        self.tdtype = torch.float64 if dtype == F64 else torch.float32
+        self.device = torch.device("cuda", torch.cuda.current_device())
+        nbytes = L.cspt_workspace_bytes(self.nx, self.ny, self.nz, int(dtype))
+        if nbytes == 0:
+            raise CsptError(EINVAL, "cspt_workspace_bytes")
+        self.workspace = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        h_ = ctypes.c_void_p()
+        bc_arr = (ctypes.c_int * 6)(*[int(b) for b in bc])
+        _check(L.cspt_create(ctypes.byref(h_), self.nx, self.ny, self.nz, float(h), float(gamma), bc_arr, int(dtype),
+                             ctypes.c_void_p(self.workspace.data_ptr()), nbytes,
+                             ctypes.c_void_p(self.stream.cuda_stream)), "cspt_create")
+        self._h = h_
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.torch.cuda.synchronize()
+            lib().cspt_destroy(self._h)
+            self._h = None
+            self.workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- helpers ---------------------------------------------------------------------
+    def _dev(self, a):
+        t = self.torch.as_tensor(a)
+        t = t.to(device=self.device, dtype=self.tdtype).contiguous()
+        assert tuple(t.shape) == self.shape, (tuple(t.shape), self.shape)
+        return t
+
+    def _host(self, a):
+        t = self.torch.as_tensor(a)
+        assert t.device.type == "cpu" and t.dtype == self.tdtype and t.is_contiguous() and tuple(t.shape) == self.shape
+        return t
+
+    def _empty(self, n, dtype=None):
+        return [self.torch.empty(self.shape, dtype=dtype or self.tdtype, device=self.device) for _ in range(n)]
+
+    # -- the C ABI, same names -----------------------------------------------------------
+    def set_state(self, rho, u, v, w, p, psi):
+        ts = [self._dev(a) for a in (rho, u, v, w, p, psi)]
+        _check(lib().cspt_set_state(self._h, *[_dptr(t) for t in ts]), "cspt_set_state")
+        self.stream.synchronize()      # inputs may be temporaries
+
+    def set_state_host(self, rho, u, v, w, p, psi):
+        ts = [self._host(a) for a in (rho, u, v, w, p, psi)]
+        _check(lib().cspt_set_state_host(self._h, *[_dptr(t) for t in ts]), "cspt_set_state_host")
+
+    def compute_dt(self, cfl):
+        out = ctypes.c_double()
+        _check(lib().cspt_compute_dt(self._h, float(cfl), ctypes.byref(out)), "cspt_compute_dt")
+        return out.value
+
+    def step(self, dt):
+        _check(lib().cspt_step(self._h, float(dt)), "cspt_step")
+
+    def step_cfl(self, cfl, want_dt=False):
+        if want_dt:
+            out = ctypes.c_double()
+            _check(lib().cspt_step_cfl(self._h, float(cfl), ctypes.byref(out)), "cspt_step_cfl")
+            return out.value
+        _check(lib().cspt_step_cfl(self._h, float(cfl), None), "cspt_step_cfl")
+        return None
+
+    def get_state(self):
+        out = self._empty(5)
+        _check(lib().cspt_get_state(self._h, *[_dptr(t) for t in out]), "cspt_get_state")
+        return out
+
+    def get_conserved(self):
+        out = self._empty(5)
+        _check(lib().cspt_get_conserved(self._h, *[_dptr(t) for t in out]), "cspt_get_conserved")
+        return out
+
+    def get_conserved_host(self, out):
+        ts = [self._host(a) for a in out]
+        _check(lib().cspt_get_conserved_host(self._h, *[_dptr(t) for t in ts]), "cspt_get_conserved_host")
+        return out
+
+    def set_conserved(self, rho, mx, my, mz, E):
+        ts = [self._dev(a) for a in (rho, mx, my, mz, E)]
+        _check(lib().cspt_set_conserved(self._h, *[_dptr(t) for t in ts]), "cspt_set_conserved")
+        self.stream.synchronize()
+
+    def get_vacuum_mask(self):
+        m = self.torch.empty(self.shape, dtype=self.torch.uint8, device=self.device)
+        _check(lib().cspt_get_vacuum_mask(self._h, _dptr(m)), "cspt_get_vacuum_mask")
+        return m
+
+    def launch_count(self):
+        return int(lib().cspt_launch_count(self._h))
+
+    def sync(self):
+        _check(lib().cspt_sync(self._h), "cspt_sync")

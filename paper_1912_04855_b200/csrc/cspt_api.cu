@@ -1,0 +1,392 @@
+// cspt_api.cu -- the C ABI declared in include/cspt.h: argument checks, workspace
+// carving and kernel launches.  All arithmetic of the method is in the kernels.
+#include <new>
+#include <string.h>
+
+#include "cspt_step.cuh"
+
+using namespace cspt;
+
+namespace {
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+size_t elem_size(int dtype) { return dtype == CSPT_F64 ? 8 : 4; }
+
+long long inflow_plane_elems(const Layout& L) {
+  long long a = (long long)L.px * L.py, b = (long long)L.py * L.pz, c = (long long)L.px * L.pz;
+  long long m = a > b ? a : b;
+  return m > c ? m : c;
+}
+
+bool valid_dims(int nx, int ny, int nz, int dtype) {
+  if (nx < 1 || ny < 1 || nz < 1) return false;
+  if (dtype != CSPT_F64 && dtype != CSPT_F32) return false;
+  Layout L = make_layout(nx, ny, nz);
+  // 32-bit cell counts inside kernels are avoided, but keep the padded field below 2^40 elements
+  return L.fstride < (1LL << 40);
+}
+
+void carve(cspt_ctx* c) {
+  size_t e = c->elem;
+  c->off_fields = 0;
+  c->inflow_plane = inflow_plane_elems(c->L);
+  c->off_inflow = align_up((size_t)S_COUNT * c->L.fstride * e, 256);
+  c->off_scalars = align_up(c->off_inflow + (size_t)6 * 5 * c->inflow_plane * e, 256);
+}
+
+template <class T> T* field(cspt_ctx* c, int slot) { return (T*)((char*)c->ws + c->off_fields) + (long long)slot * c->L.fstride; }
+template <class T> T* inflow(cspt_ctx* c, int face) { return (T*)((char*)c->ws + c->off_inflow) + (long long)face * 5 * c->inflow_plane; }
+template <class T> DevScalars<T>* scalars(cspt_ctx* c) { return (DevScalars<T>*)((char*)c->ws + c->off_scalars); }
+
+template <class T> Params<T> make_params(const cspt_ctx* c) {
+  Params<T> P;
+  P.L = c->L;
+  P.h = (T)c->h;
+  P.gamma = (T)c->gamma;
+  P.rho_vac = (T)1e-12;
+  P.inv_h = (T)1 / P.h;
+  // Monaghan cubic spline, smoothing length h: g^(q) = -W'(q)/q (G5)
+  double s2 = sqrt(2.0), s3 = sqrt(3.0);
+  double g1 = 0.75, g2 = 0.75 * (2.0 - s2) * (2.0 - s2) / s2, g3 = 0.75 * (2.0 - s3) * (2.0 - s3) / s3;
+  double S = 2.0 * g1 + 8.0 * g2 + 8.0 * g3;
+  P.a1 = (T)(g1 / S); P.a2 = (T)(g2 / S); P.a3 = (T)(g3 / S);
+  P.wnorm = (T)(1.0 / ((double)(T)S * (double)P.h * (double)P.h));
+  for (int q = 0; q < 6; ++q) P.bc[q] = c->bc[q];
+  return P;
+}
+
+inline int blocks_for(long long n, int threads, int cap = 0) {
+  long long b = (n + threads - 1) / threads;
+  if (b < 1) b = 1;
+  if (cap > 0 && b > cap) b = cap;
+  return (int)b;
+}
+
+constexpr int TPB = 256;
+constexpr int STRIDE_CAP = 148 * 16;   // grid-stride kernels: 16 CTAs of 256 threads per SM
+
+#define LAUNCH(ctx, kernel, grid, block, ...)                     \
+  do {                                                            \
+    kernel<<<(grid), (block), 0, (ctx)->stream>>>(__VA_ARGS__);   \
+    (ctx)->launches++;                                            \
+  } while (0)
+
+int check(cspt_ctx* c) {
+  if (c->cuda_error) return CSPT_ECUDA;
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { c->cuda_error = (int)e; return CSPT_ECUDA; }
+  return CSPT_OK;
+}
+
+int cuda_call(cspt_ctx* c, cudaError_t e) {
+  if (e != cudaSuccess) { c->cuda_error = (int)e; return CSPT_ECUDA; }
+  return CSPT_OK;
+}
+
+// ---- ghost layers, x then y then z (G16) ----------------------------------------------
+template <class T>
+void fill_ghosts(cspt_ctx* c, T* F, int nfields, int mode) {
+  const Layout& L = c->L;
+  int n[3] = {L.nx, L.ny, L.nz};
+  for (int d = 0; d < 3; ++d) {
+    int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+    long long e1 = d1 < d ? n[d1] + 2 * NG : n[d1], e2 = d2 < d ? n[d2] + 2 * NG : n[d2];
+    long long total = e1 * e2 * NG * 2;
+    LAUNCH(c, k_ghost_axis<T>, blocks_for(total, TPB, STRIDE_CAP), TPB, L, d, mode, c->bc[2 * d], c->bc[2 * d + 1],
+           nfields, F, inflow<T>(c, 2 * d), inflow<T>(c, 2 * d + 1), c->inflow_plane);
+  }
+}
+
+template <class T>
+int set_state_t(cspt_ctx* c, const void* rho, const void* u, const void* v, const void* w, const void* p, const void* psi) {
+  Params<T> P = make_params<T>(c);
+  long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
+  T* U = field<T>(c, S_U0);
+  T* psi_pad = field<T>(c, S_UT);          // scratch: U~ is dead between steps
+  LAUNCH(c, k_set_state<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, (const T*)rho, (const T*)u, (const T*)v,
+         (const T*)w, (const T*)p, (const T*)psi, U, psi_pad);
+  fill_ghosts<T>(c, psi_pad, 1, 2);
+  long long ne = (long long)(c->L.nx + 4) * (c->L.ny + 4) * (c->L.nz + 4);
+  LAUNCH(c, k_force<T>, blocks_for(ne, TPB, STRIDE_CAP), TPB, P, psi_pad, field<T>(c, S_F));
+  fill_ghosts<T>(c, U, 5, 1);
+  c->cur = 0;
+  c->has_state = true;
+  c->smax_valid = false;
+  return check(c);
+}
+
+template <class T>
+int set_conserved_t(cspt_ctx* c, const void* const in[5]) {
+  long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
+  T* U = field<T>(c, c->cur ? S_U1 : S_U0);
+  for (int f = 0; f < 5; ++f)
+    LAUNCH(c, k_put_field<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, c->L, (const T*)in[f], U + f * c->L.fstride);
+  c->smax_valid = false;
+  return check(c);
+}
+
+template <class T>
+int get_conserved_t(cspt_ctx* c, void* const out[5]) {
+  long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
+  const T* U = field<T>(c, c->cur ? S_U1 : S_U0);
+  for (int f = 0; f < 5; ++f)
+    LAUNCH(c, k_get_field<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, c->L, U + f * c->L.fstride, (T*)out[f]);
+  return check(c);
+}
+
+template <class T>
+int get_state_t(cspt_ctx* c, void* rho, void* u, void* v, void* w, void* p, unsigned char* mask) {
+  Params<T> P = make_params<T>(c);
+  long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
+  const T* U = field<T>(c, c->cur ? S_U1 : S_U0);
+  LAUNCH(c, k_get_state<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, U, (T*)rho, (T*)u, (T*)v, (T*)w, (T*)p, mask);
+  return check(c);
+}
+
+template <class T>
+void ensure_smax(cspt_ctx* c) {
+  if (c->smax_valid) return;
+  Params<T> P = make_params<T>(c);
+  long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
+  LAUNCH(c, k_reset_smax<T>, 1, 1, scalars<T>(c));
+  LAUNCH(c, k_speed_max<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, field<T>(c, c->cur ? S_U1 : S_U0),
+         &scalars<T>(c)->smax_bits);
+  c->smax_valid = true;
+}
+
+template <class T>
+int compute_dt_t(cspt_ctx* c, double cfl, double* out) {
+  typedef typename Real<T>::bits_t bits_t;
+  ensure_smax<T>(c);
+  int rc = check(c);
+  if (rc) return rc;
+  bits_t* hb = (bits_t*)c->h_pinned;
+  rc = cuda_call(c, cudaMemcpyAsync(hb, &scalars<T>(c)->smax_bits, sizeof(bits_t), cudaMemcpyDeviceToHost, c->stream));
+  if (rc) return rc;
+  rc = cuda_call(c, cudaStreamSynchronize(c->stream));
+  if (rc) return rc;
+  T smax;
+  memcpy(&smax, hb, sizeof(T));
+  // same two rn operations as k_dt_finalize and the oracle: (cfl*h)/smax in T
+  volatile T num = (T)cfl * (T)c->h;
+  T dt = smax > (T)0 ? (T)(num / smax) : Real<T>::inf();
+  *out = (double)dt;
+  return CSPT_OK;
+}
+
+template <class T>
+void run_step(cspt_ctx* c) {
+  Params<T> P = make_params<T>(c);
+  const Layout& L = c->L;
+  T* U = field<T>(c, c->cur ? S_U1 : S_U0);
+  T* UN = field<T>(c, c->cur ? S_U0 : S_U1);
+  DevScalars<T>* sc = scalars<T>(c);
+  fill_ghosts<T>(c, U, 5, 0);                                                      // O0
+  long long n3 = (long long)(L.nx + 6) * (L.ny + 6) * (L.nz + 6);
+  long long n2 = (long long)(L.nx + 4) * (L.ny + 4) * (L.nz + 4);
+  long long n1 = (long long)(L.nx + 2) * (L.ny + 2) * (L.nz + 2);
+  long long n0 = (long long)L.nx * L.ny * L.nz;
+  LAUNCH(c, k_prim<T>, blocks_for(n3, TPB), TPB, P, U, field<T>(c, S_PR));          // O1
+  LAUNCH(c, k_predictor<T>, blocks_for(n2, TPB), TPB, P, sc, U, field<T>(c, S_PR), field<T>(c, S_F),
+         field<T>(c, S_US), field<T>(c, S_PS));                                    // O3, O4
+  LAUNCH(c, k_corrector<T>, blocks_for(n1, TPB), TPB, P, sc, U, field<T>(c, S_PR), field<T>(c, S_F),
+         field<T>(c, S_US), field<T>(c, S_PS), field<T>(c, S_UT), field<T>(c, S_XI));   // O5, O6
+  LAUNCH(c, k_reset_smax<T>, 1, 1, sc);
+  LAUNCH(c, k_euler<T>, blocks_for(n0, TPB), TPB, P, sc, U, field<T>(c, S_UT), field<T>(c, S_XI), UN,
+         &sc->smax_bits);                                                          // O7, O8 (+O9 epilogue)
+  c->cur ^= 1;
+  c->smax_valid = true;
+}
+
+template <class T>
+int step_t(cspt_ctx* c, double dt) {
+  LAUNCH(c, k_set_dt<T>, 1, 1, scalars<T>(c), (T)dt);
+  run_step<T>(c);
+  return check(c);
+}
+
+template <class T>
+int step_cfl_t(cspt_ctx* c, double cfl, double* out) {
+  ensure_smax<T>(c);
+  LAUNCH(c, k_dt_finalize<T>, 1, 1, scalars<T>(c), (T)cfl, (T)c->h);
+  run_step<T>(c);
+  int rc = check(c);
+  if (rc || !out) return rc;
+  T* hb = (T*)c->h_pinned;
+  rc = cuda_call(c, cudaMemcpyAsync(hb, &scalars<T>(c)->dt, sizeof(T), cudaMemcpyDeviceToHost, c->stream));
+  if (rc) return rc;
+  rc = cuda_call(c, cudaStreamSynchronize(c->stream));
+  if (rc) return rc;
+  *out = (double)*hb;
+  return CSPT_OK;
+}
+
+// dense staging arrays for the *_host entry points live in the (dead between steps)
+// intermediate slots S_PR.. (12 padded slots >= 6 dense arrays)
+template <class T> T* staging(cspt_ctx* c, int f) { return field<T>(c, S_PR + f); }
+
+}  // namespace
+
+#define DISPATCH(c, call) ((c)->dtype == CSPT_F64 ? call<double> : call<float>)
+
+extern "C" {
+
+size_t cspt_workspace_bytes(int nx, int ny, int nz, int dtype) {
+  if (!valid_dims(nx, ny, nz, dtype)) return 0;
+  cspt_ctx tmp;
+  tmp.L = make_layout(nx, ny, nz);
+  tmp.elem = elem_size(dtype);
+  carve(&tmp);
+  return tmp.off_scalars + 256;
+}
+
+int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, const int bc[6], int dtype,
+                void* workspace, size_t workspace_bytes, void* cuda_stream) {
+  if (!out) return CSPT_EINVAL;
+  *out = nullptr;
+  if (!bc || !workspace || !valid_dims(nx, ny, nz, dtype)) return CSPT_EINVAL;
+  if (!(h > 0) || !(gamma > 1) || !isfinite(h) || !isfinite(gamma)) return CSPT_EINVAL;
+  int n[3] = {nx, ny, nz};
+  for (int d = 0; d < 3; ++d) {
+    int lo = bc[2 * d], hi = bc[2 * d + 1];
+    if (lo < 0 || lo > 2 || hi < 0 || hi > 2) return CSPT_EINVAL;
+    if ((lo == CSPT_BC_PERIODIC) != (hi == CSPT_BC_PERIODIC)) return CSPT_EINVAL;
+    if (lo != CSPT_BC_PERIODIC && n[d] < 4) return CSPT_EINVAL;
+  }
+  if (((uintptr_t)workspace & 255) != 0) return CSPT_EINVAL;
+  if (workspace_bytes < cspt_workspace_bytes(nx, ny, nz, dtype)) return CSPT_EINVAL;
+  cspt_ctx* c = new (std::nothrow) cspt_ctx;
+  if (!c) return CSPT_ENOMEM;
+  memset(c, 0, sizeof(*c));
+  c->L = make_layout(nx, ny, nz);
+  c->dtype = dtype;
+  c->elem = elem_size(dtype);
+  for (int q = 0; q < 6; ++q) c->bc[q] = bc[q];
+  c->h = h; c->gamma = gamma;
+  c->ws = workspace; c->ws_bytes = workspace_bytes;
+  c->stream = (cudaStream_t)cuda_stream;
+  carve(c);
+  if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
+  *out = c;
+  return CSPT_OK;
+}
+
+void cspt_destroy(cspt_ctx* c) {
+  if (!c) return;
+  if (c->h_pinned) cudaFreeHost(c->h_pinned);
+  delete c;
+}
+
+int cspt_set_state(cspt_ctx* c, const void* rho, const void* u, const void* v, const void* w, const void* p,
+                   const void* psi) {
+  if (!c || !rho || !u || !v || !w || !p || !psi) return CSPT_EINVAL;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, set_state_t)(c, rho, u, v, w, p, psi);
+}
+
+int cspt_set_state_host(cspt_ctx* c, const void* rho, const void* u, const void* v, const void* w, const void* p,
+                        const void* psi) {
+  if (!c || !rho || !u || !v || !w || !p || !psi) return CSPT_EINVAL;
+  if (c->cuda_error) return CSPT_ECUDA;
+  const void* in[6] = {rho, u, v, w, p, psi};
+  void* dev[6];
+  size_t bytes = (size_t)c->L.nx * c->L.ny * c->L.nz * c->elem;
+  for (int f = 0; f < 6; ++f) {
+    dev[f] = c->dtype == CSPT_F64 ? (void*)staging<double>(c, f) : (void*)staging<float>(c, f);
+    int rc = cuda_call(c, cudaMemcpyAsync(dev[f], in[f], bytes, cudaMemcpyHostToDevice, c->stream));
+    if (rc) return rc;
+  }
+  int rc = DISPATCH(c, set_state_t)(c, dev[0], dev[1], dev[2], dev[3], dev[4], dev[5]);
+  if (rc) return rc;
+  return cuda_call(c, cudaStreamSynchronize(c->stream));
+}
+
+int cspt_compute_dt(cspt_ctx* c, double cfl, double* dt_host_out) {
+  if (!c || !dt_host_out || !(cfl > 0) || !isfinite(cfl)) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, compute_dt_t)(c, cfl, dt_host_out);
+}
+
+int cspt_step(cspt_ctx* c, double dt) {
+  if (!c || !(dt > 0) || !isfinite(dt)) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, step_t)(c, dt);
+}
+
+int cspt_step_cfl(cspt_ctx* c, double cfl, double* dt_host_out) {
+  if (!c || !(cfl > 0) || !isfinite(cfl)) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, step_cfl_t)(c, cfl, dt_host_out);
+}
+
+int cspt_get_state(cspt_ctx* c, void* rho, void* u, void* v, void* w, void* p) {
+  if (!c || !rho || !u || !v || !w || !p) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, get_state_t)(c, rho, u, v, w, p, nullptr);
+}
+
+int cspt_get_conserved(cspt_ctx* c, void* rho, void* mx, void* my, void* mz, void* E) {
+  if (!c || !rho || !mx || !my || !mz || !E) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  void* out[5] = {rho, mx, my, mz, E};
+  return DISPATCH(c, get_conserved_t)(c, out);
+}
+
+int cspt_get_conserved_host(cspt_ctx* c, void* rho, void* mx, void* my, void* mz, void* E) {
+  if (!c || !rho || !mx || !my || !mz || !E) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  void* host[5] = {rho, mx, my, mz, E};
+  void* dev[5];
+  for (int f = 0; f < 5; ++f) dev[f] = c->dtype == CSPT_F64 ? (void*)staging<double>(c, f) : (void*)staging<float>(c, f);
+  int rc = DISPATCH(c, get_conserved_t)(c, dev);
+  if (rc) return rc;
+  size_t bytes = (size_t)c->L.nx * c->L.ny * c->L.nz * c->elem;
+  for (int f = 0; f < 5; ++f) {
+    rc = cuda_call(c, cudaMemcpyAsync(host[f], dev[f], bytes, cudaMemcpyDeviceToHost, c->stream));
+    if (rc) return rc;
+  }
+  return cuda_call(c, cudaStreamSynchronize(c->stream));
+}
+
+int cspt_set_conserved(cspt_ctx* c, const void* rho, const void* mx, const void* my, const void* mz, const void* E) {
+  if (!c || !rho || !mx || !my || !mz || !E) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  const void* in[5] = {rho, mx, my, mz, E};
+  return DISPATCH(c, set_conserved_t)(c, in);
+}
+
+int cspt_get_vacuum_mask(cspt_ctx* c, unsigned char* mask) {
+  if (!c || !mask) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, get_state_t)(c, nullptr, nullptr, nullptr, nullptr, nullptr, mask);
+}
+
+long long cspt_launch_count(const cspt_ctx* c) { return c ? c->launches : 0; }
+
+int cspt_sync(cspt_ctx* c) {
+  if (!c) return CSPT_EINVAL;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return cuda_call(c, cudaStreamSynchronize(c->stream));
+}
+
+const char* cspt_strerror(int code) {
+  switch (code) {
+    case CSPT_OK: return "ok";
+    case CSPT_EINVAL: return "invalid argument";
+    case CSPT_ENOMEM: return "out of host memory";
+    case CSPT_ECUDA: return "CUDA error (sticky until destroy)";
+    case CSPT_ESTATE: return "no state set";
+    default: return "unknown status";
+  }
+}
+
+}  // extern "C"

@@ -1,0 +1,105 @@
+// cspt_common.cuh -- grid layout, context and small device helpers of the
+// CUDA CSPH-TVD path (sm_100a).  No code is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <math.h>
+
+#include "cspt.h"
+
+namespace cspt {
+
+// Ghost layers per face: one full step reaches +-3 cells (predictor radius 1 ->
+// corrector radius 1 -> TVD stage needs U~ at +-1 and U^n at +-2).
+constexpr int NG = 3;
+// Left pad along x is 4 elements so that interior cell i = 0 sits on a 16-byte
+// (fp32) / 32-byte (fp64) boundary; the x pitch is a multiple of 16 elements.
+constexpr int GX = 4;
+
+struct Layout {
+  int nx, ny, nz;      // interior
+  int px, py, pz;      // padded (allocated) extents
+  long long fstride;   // elements per padded field
+  __host__ __device__ long long idx(int i, int j, int k) const {
+    return ((long long)(k + NG) * py + (j + NG)) * px + (i + GX);
+  }
+  __host__ __device__ long long sy() const { return px; }
+  __host__ __device__ long long sz() const { return (long long)px * py; }
+};
+
+inline Layout make_layout(int nx, int ny, int nz) {
+  Layout L;
+  L.nx = nx; L.ny = ny; L.nz = nz;
+  L.px = ((nx + GX + NG + 15) / 16) * 16;
+  L.py = ny + 2 * NG;
+  L.pz = nz + 2 * NG;
+  long long n = (long long)L.px * L.py * L.pz;
+  L.fstride = ((n + 63) / 64) * 64;
+  return L;
+}
+
+// Field slots inside the workspace (each fstride elements of T).
+enum Slot {
+  S_U0 = 0,        // U buffer A: rho, mx, my, mz, E          (5)
+  S_U1 = 5,        // U buffer B                                 (5)
+  S_F = 10,        // f = -D[psi]                                (3)
+  S_UT = 13,       // U~: mx, my, mz, E  (rho~ = rho^n, G2)      (4)
+  S_XI = 17,       // xi^{n+1}                                   (3)
+  S_PR = 20,       // primitives of U^n: phi, u, v, w            (4)
+  S_US = 24,       // U*: mx, my, mz, E                          (4)
+  S_PS = 28,       // primitives of U*: phi, u, v, w             (4)
+  S_COUNT = 32
+};
+
+template <class T> struct Real;
+template <> struct Real<double> {
+  typedef unsigned long long bits_t;
+  static __device__ __forceinline__ double mul(double a, double b) { return __dmul_rn(a, b); }
+  static __device__ __forceinline__ double add(double a, double b) { return __dadd_rn(a, b); }
+  static __device__ __forceinline__ double sub(double a, double b) { return __dadd_rn(a, -b); }
+  static __device__ __forceinline__ double div(double a, double b) { return __ddiv_rn(a, b); }
+  static __device__ __forceinline__ double sqrt(double a) { return __dsqrt_rn(a); }
+  static __device__ __forceinline__ bits_t bits(double a) { return (bits_t)__double_as_longlong(a); }
+  static __device__ __forceinline__ double from_bits(bits_t b) { return __longlong_as_double((long long)b); }
+  static __host__ __device__ __forceinline__ double inf() { return HUGE_VAL; }
+};
+template <> struct Real<float> {
+  typedef unsigned int bits_t;
+  static __device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
+  static __device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b); }
+  static __device__ __forceinline__ float sub(float a, float b) { return __fadd_rn(a, -b); }
+  static __device__ __forceinline__ float div(float a, float b) { return __fdiv_rn(a, b); }
+  static __device__ __forceinline__ float sqrt(float a) { return __fsqrt_rn(a); }
+  static __device__ __forceinline__ bits_t bits(float a) { return __float_as_uint(a); }
+  static __device__ __forceinline__ float from_bits(bits_t b) { return __uint_as_float(b); }
+  static __host__ __device__ __forceinline__ float inf() { return HUGE_VALF; }
+};
+
+// Per-step scalars living on the device, so that a step never needs the host.
+template <class T> struct DevScalars {
+  T dt;                                  // time step of the step being enqueued
+  typename Real<T>::bits_t smax_bits;    // max signal speed, IEEE bits (positive floats order like integers)
+};
+
+}  // namespace cspt
+
+struct cspt_ctx {
+  cspt::Layout L;
+  int dtype;
+  int bc[6];
+  double h, gamma;
+  void* ws;
+  size_t ws_bytes;
+  cudaStream_t stream;
+  int cur;                 // which U buffer holds U^n
+  bool has_state;
+  bool smax_valid;         // smax_bits on the device belongs to the current U^n
+  int cuda_error;          // sticky
+  long long launches;
+  void* h_pinned;          // small pinned staging buffer (scalars)
+  size_t elem;             // sizeof(T)
+  // workspace sub-buffers (byte offsets)
+  size_t off_fields, off_inflow, off_scalars;
+  long long inflow_plane;  // elements per captured plane
+};

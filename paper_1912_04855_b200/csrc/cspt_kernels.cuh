@@ -1,0 +1,266 @@
+// cspt_kernels.cuh -- device code of the CSPH-TVD step (sm_100a).
+// Citations are to /root/reference/PAPER.md (section 2.2) and to the readings
+// G1..G23 of DESIGN.md section 3.
+#pragma once
+#include "cspt_common.cuh"
+
+namespace cspt {
+
+template <class T> struct Params {
+  Layout L;
+  T h, gamma, rho_vac;
+  T inv_h;
+  T a1, a2, a3;     // lattice weights a(|o|^2) of the undisplaced cubic-spline operator (G5)
+  T wnorm;          // 1 / (S0' h^2): kernel weight normalisation (G5)
+  int bc[6];
+};
+
+// ---- primitives of one cell (G7, G9) ----------------------------
+template <class T> struct Prim { T u, v, w, p, phi; bool ok; };
+
+// Exactly rounded version: every operation is a single IEEE rn operation in a fixed
+// order, so that the CFL time step and the vacuum mask are bit-exact (G15).
+template <class T>
+__device__ __forceinline__ Prim<T> prim_exact(T rho, T mx, T my, T mz, T E, T gamma, T rho_vac) {
+  typedef Real<T> R;
+  Prim<T> q;
+  q.ok = rho > rho_vac;
+  T ir = q.ok ? R::div((T)1, rho) : (T)0;
+  q.u = R::mul(mx, ir); q.v = R::mul(my, ir); q.w = R::mul(mz, ir);
+  T ke2 = R::add(R::add(R::mul(mx, q.u), R::mul(my, q.v)), R::mul(mz, q.w));
+  T pp = R::mul(R::sub(gamma, (T)1), R::sub(E, R::mul((T)0.5, ke2)));
+  q.p = q.ok ? (pp > (T)0 ? pp : (T)0) : (T)0;
+  q.phi = R::sqrt(R::mul((T)2, q.p));
+  return q;
+}
+
+// Fast version for the step kernels (contraction allowed; parity is to 1e-11 / 1e-4).
+template <class T>
+__device__ __forceinline__ Prim<T> prim_fast(T rho, T mx, T my, T mz, T E, T gamma, T rho_vac) {
+  Prim<T> q;
+  q.ok = rho > rho_vac;
+  T ir = q.ok ? (T)1 / rho : (T)0;
+  q.u = mx * ir; q.v = my * ir; q.w = mz * ir;
+  T ke2 = (mx * q.u + my * q.v) + mz * q.w;
+  T pp = (gamma - (T)1) * (E - (T)0.5 * ke2);
+  q.p = q.ok ? (pp > (T)0 ? pp : (T)0) : (T)0;
+  q.phi = sqrt((T)2 * q.p);
+  return q;
+}
+
+// ---- set_state: primitives -> conserved, psi into a scratch field ----
+template <class T>
+__global__ void k_set_state(Params<T> P, const T* __restrict__ rho, const T* __restrict__ u,
+                            const T* __restrict__ v, const T* __restrict__ w, const T* __restrict__ p,
+                            const T* __restrict__ psi, T* __restrict__ U, T* __restrict__ psi_pad) {
+  typedef Real<T> R;
+  const Layout& L = P.L;
+  long long n = (long long)L.nx * L.ny * L.nz;
+  for (long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) {
+    int i = (int)(m % L.nx);
+    long long r = m / L.nx;
+    int j = (int)(r % L.ny), k = (int)(r / L.ny);
+    long long c = L.idx(i, j, k);
+    T ro = rho[m], uu = u[m], vv = v[m], ww = w[m];
+    U[c] = ro;
+    U[c + L.fstride] = R::mul(ro, uu);
+    U[c + 2 * L.fstride] = R::mul(ro, vv);
+    U[c + 3 * L.fstride] = R::mul(ro, ww);
+    T ke = R::add(R::add(R::mul(uu, uu), R::mul(vv, vv)), R::mul(ww, ww));
+    U[c + 4 * L.fstride] = R::add(R::div(p[m], R::sub(P.gamma, (T)1)), R::mul(R::mul((T)0.5, ro), ke));
+    if (psi_pad) psi_pad[c] = psi[m];
+  }
+}
+
+template <class T>
+__global__ void k_put_field(Layout L, const T* __restrict__ src, T* __restrict__ dst) {
+  long long n = (long long)L.nx * L.ny * L.nz;
+  for (long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) {
+    int i = (int)(m % L.nx);
+    long long r = m / L.nx;
+    dst[L.idx(i, (int)(r % L.ny), (int)(r / L.ny))] = src[m];
+  }
+}
+
+template <class T>
+__global__ void k_get_field(Layout L, const T* __restrict__ src, T* __restrict__ dst) {
+  long long n = (long long)L.nx * L.ny * L.nz;
+  for (long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) {
+    int i = (int)(m % L.nx);
+    long long r = m / L.nx;
+    dst[m] = src[L.idx(i, (int)(r % L.ny), (int)(r / L.ny))];
+  }
+}
+
+template <class T>
+__global__ void k_get_state(Params<T> P, const T* __restrict__ U, T* __restrict__ rho, T* __restrict__ u,
+                            T* __restrict__ v, T* __restrict__ w, T* __restrict__ p, unsigned char* __restrict__ mask) {
+  const Layout& L = P.L;
+  long long n = (long long)L.nx * L.ny * L.nz;
+  for (long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) {
+    int i = (int)(m % L.nx);
+    long long r = m / L.nx;
+    long long c = L.idx(i, (int)(r % L.ny), (int)(r / L.ny));
+    T ro = U[c];
+    if (mask) { mask[m] = ro > P.rho_vac ? 0 : 1; continue; }
+    Prim<T> q = prim_exact<T>(ro, U[c + L.fstride], U[c + 2 * L.fstride], U[c + 3 * L.fstride], U[c + 4 * L.fstride], P.gamma, P.rho_vac);
+    rho[m] = ro; u[m] = q.u; v[m] = q.v; w[m] = q.w; p[m] = q.p;
+  }
+}
+
+// ---- O0: ghost layers along one axis (G16) ----------------------------------------
+// mode 0: state fields (wrap / copy boundary cell / frozen inflow layer)
+// mode 1: like 0 but INFLOW faces are filled like OUTFLOW and their layer is captured
+// mode 2: potential (wrap / odd reflection about the boundary cell)
+// Axes before `d` are traversed over their padded range, axes after it over the interior,
+// so that x, y, z launches in this order fill edges and corners.
+template <class T>
+__global__ void k_ghost_axis(Layout L, int d, int mode, int bc_lo, int bc_hi, int nfields,
+                             T* __restrict__ F, T* __restrict__ inflow_lo, T* __restrict__ inflow_hi,
+                             long long inflow_plane) {
+  int n[3] = {L.nx, L.ny, L.nz};
+  int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
+  int lo1 = d1 < d ? -NG : 0, hi1 = d1 < d ? n[d1] + NG : n[d1];
+  int lo2 = d2 < d ? -NG : 0, hi2 = d2 < d ? n[d2] + NG : n[d2];
+  long long e1 = hi1 - lo1, e2 = hi2 - lo2;
+  long long total = e1 * e2 * NG * 2;
+  for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+    // fastest index: along the axis that is contiguous in memory when possible
+    long long r = t;
+    int b, a, g, side;
+    if (d == 0) { g = (int)(r % NG) + 1; r /= NG; side = (int)(r % 2); r /= 2; b = (int)(r % e1) + lo1; a = (int)(r / e1) + lo2; }
+    else if (d == 1) { a = (int)(r % e2) + lo2; r /= e2; g = (int)(r % NG) + 1; r /= NG; side = (int)(r % 2); r /= 2; b = (int)r + lo1; }
+    else { b = (int)(r % e1) + lo1; r /= e1; a = (int)(r % e2) + lo2; r /= e2; g = (int)(r % NG) + 1; side = (int)(r / NG); }
+    int kind = side ? bc_hi : bc_lo;
+    int q[3], s[3], e0[3];
+    q[d1] = b; q[d2] = a; s[d1] = b; s[d2] = a; e0[d1] = b; e0[d2] = a;
+    q[d] = side ? n[d] - 1 + g : -g;
+    e0[d] = side ? n[d] - 1 : 0;
+    long long cq = L.idx(q[0], q[1], q[2]);
+    if (kind == CSPT_BC_PERIODIC) {
+      s[d] = side ? ((g - 1) % n[d]) : (n[d] - 1 - ((g - 1) % n[d]));
+      long long cs = L.idx(s[0], s[1], s[2]);
+      for (int f = 0; f < nfields; ++f) F[cq + f * L.fstride] = F[cs + f * L.fstride];
+    } else if (mode == 2) {
+      s[d] = side ? n[d] - 1 - g : g;
+      s[d] = max(0, min(n[d] - 1, s[d]));
+      long long cs = L.idx(s[0], s[1], s[2]), ce = L.idx(e0[0], e0[1], e0[2]);
+      F[cq] = (T)2 * F[ce] - F[cs];
+    } else {
+      long long ce = L.idx(e0[0], e0[1], e0[2]);
+      // captured planes are indexed by the padded coordinates of the two other axes
+      int pd1 = d1 == 0 ? L.px : (d1 == 1 ? L.py : L.pz);
+      int off1 = d1 == 0 ? GX : NG, off2 = d2 == 0 ? GX : NG;
+      long long pi = (long long)(a + off2) * pd1 + (b + off1);
+      T* inf = side ? inflow_hi : inflow_lo;
+      for (int f = 0; f < nfields; ++f) {
+        T val;
+        if (kind == CSPT_BC_INFLOW && mode == 0) val = inf[f * inflow_plane + pi];
+        else val = F[ce + f * L.fstride];
+        F[cq + f * L.fstride] = val;
+        if (kind == CSPT_BC_INFLOW && mode == 1 && g == 1) inf[f * inflow_plane + pi] = val;
+      }
+    }
+  }
+}
+
+// ---- O2: external force f = -D[psi] on interior(+)2 (G5, G6) -----
+template <class T>
+__global__ void k_force(Params<T> P, const T* __restrict__ psi, T* __restrict__ F) {
+  const Layout& L = P.L;
+  int ex = L.nx + 4, ey = L.ny + 4, ez = L.nz + 4;
+  long long n = (long long)ex * ey * ez;
+  for (long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) {
+    int i = (int)(m % ex) - 2;
+    long long r = m / ex;
+    int j = (int)(r % ey) - 2, k = (int)(r / ey) - 2;
+    long long c = L.idx(i, j, k);
+    T s0 = 0, s1 = 0, s2 = 0;
+#pragma unroll
+    for (int oz = -1; oz <= 1; ++oz)
+#pragma unroll
+      for (int oy = -1; oy <= 1; ++oy)
+#pragma unroll
+        for (int ox = -1; ox <= 1; ++ox) {
+          int o2 = ox * ox + oy * oy + oz * oz;
+          if (o2 == 0) continue;
+          T a = o2 == 1 ? P.a1 : (o2 == 2 ? P.a2 : P.a3);
+          T q = a * psi[c + oz * L.sz() + oy * L.sy() + ox];
+          s0 += (T)ox * q; s1 += (T)oy * q; s2 += (T)oz * q;
+        }
+    F[c] = -(s0 / P.h);
+    F[c + L.fstride] = -(s1 / P.h);
+    F[c + 2 * L.fstride] = -(s2 / P.h);
+  }
+}
+
+// ---- O9: CFL signal speed maximum (paper silent; G15) -----------------------------
+// Per-thread max -> warp shuffle max -> block max -> integer atomicMax on the IEEE bit
+// pattern (non-negative floats order like unsigned integers): bit-exact, order independent.
+template <class T>
+__device__ __forceinline__ T cell_speed_exact(T rho, T mx, T my, T mz, T E, T gamma, T rho_vac) {
+  typedef Real<T> R;
+  Prim<T> q = prim_exact<T>(rho, mx, my, mz, E, gamma, rho_vac);
+  if (!q.ok) return (T)0;
+  T cs = R::sqrt(R::div(R::mul(gamma, q.p), rho));
+  T a = fabs(q.u), b = fabs(q.v), c = fabs(q.w);
+  T m = a > b ? a : b;
+  m = m > c ? m : c;
+  return R::add(cs, m);
+}
+
+template <class T>
+__device__ __forceinline__ void block_max_to_global(T s, typename Real<T>::bits_t* out) {
+  typedef typename Real<T>::bits_t bits_t;
+  __shared__ bits_t sm[32];
+  bits_t b = s > (T)0 ? Real<T>::bits(s) : (bits_t)0;      // NaN and 0 contribute nothing
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    bits_t other = __shfl_xor_sync(0xffffffffu, b, o);
+    b = other > b ? other : b;
+  }
+  int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) sm[wid] = b;
+  __syncthreads();
+  if (wid == 0) {
+    int nw = (blockDim.x * blockDim.y * blockDim.z + 31) >> 5;
+    b = lane < nw ? sm[lane] : (bits_t)0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      bits_t other = __shfl_xor_sync(0xffffffffu, b, o);
+      b = other > b ? other : b;
+    }
+    if (lane == 0 && b != 0) atomicMax(out, b);
+  }
+}
+
+template <class T>
+__global__ void k_speed_max(Params<T> P, const T* __restrict__ U, typename Real<T>::bits_t* out) {
+  const Layout& L = P.L;
+  long long n = (long long)L.nx * L.ny * L.nz;
+  T smax = 0;
+  for (long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) {
+    int i = (int)(m % L.nx);
+    long long r = m / L.nx;
+    long long c = L.idx(i, (int)(r % L.ny), (int)(r / L.ny));
+    T s = cell_speed_exact<T>(U[c], U[c + L.fstride], U[c + 2 * L.fstride], U[c + 3 * L.fstride], U[c + 4 * L.fstride], P.gamma, P.rho_vac);
+    if (s > smax) smax = s;
+  }
+  block_max_to_global<T>(smax, out);
+}
+
+// dt = (cfl*h)/smax in T, one rn operation each: identical to the host formula.
+template <class T>
+__global__ void k_dt_finalize(DevScalars<T>* sc, T cfl, T h) {
+  typedef Real<T> R;
+  T smax = R::from_bits(sc->smax_bits);
+  sc->dt = smax > (T)0 ? R::div(R::mul(cfl, h), smax) : R::inf();
+}
+
+template <class T>
+__global__ void k_set_dt(DevScalars<T>* sc, T dt) { sc->dt = dt; }
+
+template <class T>
+__global__ void k_reset_smax(DevScalars<T>* sc) { sc->smax_bits = 0; }
+
+}  // namespace cspt

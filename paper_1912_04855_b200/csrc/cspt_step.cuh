@@ -1,0 +1,212 @@
+// cspt_step.cuh -- the step kernels: HFC/SUL predictor, HFC/SUL corrector, FGC+SUE.
+// (Eq. (4)-(8)).  First, straightforward version: one thread per
+// cell, stencil operands read through L1/L2.
+#pragma once
+#include "cspt_kernels.cuh"
+
+namespace cspt {
+
+// decode a linear index over the box [-ext, n+ext)^3
+__device__ __forceinline__ bool decode_ext(const Layout& L, int ext, long long m, int& i, int& j, int& k) {
+  int ex = L.nx + 2 * ext, ey = L.ny + 2 * ext, ez = L.nz + 2 * ext;
+  if (m >= (long long)ex * ey * ez) return false;
+  i = (int)(m % ex) - ext;
+  long long r = m / ex;
+  j = (int)(r % ey) - ext;
+  k = (int)(r / ey) - ext;
+  return true;
+}
+
+template <class T>
+__device__ __forceinline__ T load_dt(const DevScalars<T>* sc) {
+  T dt = sc->dt;
+  return dt < Real<T>::inf() ? dt : (T)0;       // all-vacuum grid: dt = +inf -> identity step
+}
+
+// O1 on the whole padded array: phi, u, v, w of U^n.
+template <class T>
+__global__ void k_prim(Params<T> P, const T* __restrict__ U, T* __restrict__ PR) {
+  const Layout& L = P.L;
+  long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  int i, j, k;
+  if (!decode_ext(L, NG, m, i, j, k)) return;
+  long long c = L.idx(i, j, k), fs = L.fstride;
+  Prim<T> q = prim_fast<T>(U[c], U[c + fs], U[c + 2 * fs], U[c + 3 * fs], U[c + 4 * fs], P.gamma, P.rho_vac);
+  PR[c] = q.phi; PR[c + fs] = q.u; PR[c + 2 * fs] = q.v; PR[c + 3 * fs] = q.w;
+}
+
+// O3+O4: HFC{predictor} + SUL{predictor}, Eq. (7) with particles at the cell centres
+// and Eq. (5), on interior(+)2.
+template <class T>
+__global__ void k_predictor(Params<T> P, const DevScalars<T>* sc, const T* __restrict__ U, const T* __restrict__ PR,
+                            const T* __restrict__ F, T* __restrict__ US, T* __restrict__ PS) {
+  const Layout& L = P.L;
+  long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  int i, j, k;
+  if (!decode_ext(L, 2, m, i, j, k)) return;
+  T dt = load_dt(sc);
+  long long c = L.idx(i, j, k), fs = L.fstride;
+  T ui = PR[c + fs], vi = PR[c + 2 * fs], wi = PR[c + 3 * fs], phi_i = PR[c];
+  T sx = 0, sy = 0, sz = 0, se = 0;
+#pragma unroll
+  for (int oz = -1; oz <= 1; ++oz)
+#pragma unroll
+    for (int oy = -1; oy <= 1; ++oy)
+#pragma unroll
+      for (int ox = -1; ox <= 1; ++ox) {
+        int o2 = ox * ox + oy * oy + oz * oz;
+        if (o2 == 0) continue;
+        T a = o2 == 1 ? P.a1 : (o2 == 2 ? P.a2 : P.a3);
+        long long cj = c + oz * L.sz() + oy * L.sy() + ox;
+        T pw = PR[cj] * a;                      // phi_j * a(|o|^2); d = -o h
+        T ud = (T)0;
+        if (ox) { sx -= (T)ox * pw; ud -= (T)ox * (ui + PR[cj + fs]); }
+        if (oy) { sy -= (T)oy * pw; ud -= (T)oy * (vi + PR[cj + 2 * fs]); }
+        if (oz) { sz -= (T)oz * pw; ud -= (T)oz * (wi + PR[cj + 3 * fs]); }
+        se += pw * ud;
+      }
+  T rho = U[c];
+  T fx = F[c], fy = F[c + fs], fz = F[c + 2 * fs];
+  // S = (1/h) * sum a o phi_j  (sign folded above); Q per G1
+  T qx = phi_i * sx * P.inv_h + rho * fx;
+  T qy = phi_i * sy * P.inv_h + rho * fy;
+  T qz = phi_i * sz * P.inv_h + rho * fz;
+  T qe = phi_i * se * ((T)0.5 * P.inv_h) + rho * ((ui * fx + vi * fy) + wi * fz);
+  T mx = U[c + fs] + dt * qx, my = U[c + 2 * fs] + dt * qy, mz = U[c + 3 * fs] + dt * qz, E = U[c + 4 * fs] + dt * qe;
+  US[c] = mx; US[c + fs] = my; US[c + 2 * fs] = mz; US[c + 3 * fs] = E;
+  Prim<T> q = prim_fast<T>(rho, mx, my, mz, E, P.gamma, P.rho_vac);
+  PS[c] = q.phi; PS[c + fs] = q.u; PS[c + 2 * fs] = q.v; PS[c + 3 * fs] = q.w;
+}
+
+// -W'(q)/q of the Monaghan cubic spline with smoothing length h (G5).
+template <class T>
+__device__ __forceinline__ T spline_g(T qq) {
+  T t = (T)2 - qq;
+  T g1 = (T)3 - (T)2.25 * qq;
+  T g2 = (T)0.75 * t * t / qq;
+  return qq < (T)1 ? g1 : (qq < (T)2 ? g2 : (T)0);
+}
+
+// O5/O6: HFC{corrector} + SUL{corrector}, Eq. (7) at displaced positions r* and Eq. (6),
+// on interior(+)1.  xi* = dt/2 (u^n + u*) is formed on the fly (Eq. (5), r^n = centre).
+template <class T>
+__global__ void k_corrector(Params<T> P, const DevScalars<T>* sc, const T* __restrict__ U, const T* __restrict__ PR,
+                            const T* __restrict__ F, const T* __restrict__ US, const T* __restrict__ PS,
+                            T* __restrict__ UT, T* __restrict__ XI) {
+  const Layout& L = P.L;
+  long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  int i, j, k;
+  if (!decode_ext(L, 1, m, i, j, k)) return;
+  T dt = load_dt(sc);
+  T hdt = (T)0.5 * dt;
+  long long c = L.idx(i, j, k), fs = L.fstride;
+  T un = PR[c + fs], vn = PR[c + 2 * fs], wn = PR[c + 3 * fs];
+  T ui = PS[c + fs], vi = PS[c + 2 * fs], wi = PS[c + 3 * fs], phi_i = PS[c];
+  T xix = hdt * (un + ui), xiy = hdt * (vn + vi), xiz = hdt * (wn + wi);
+  T sx = 0, sy = 0, sz = 0, se = 0;
+#pragma unroll
+  for (int oz = -1; oz <= 1; ++oz)
+#pragma unroll
+    for (int oy = -1; oy <= 1; ++oy)
+#pragma unroll
+      for (int ox = -1; ox <= 1; ++ox) {
+        if (ox == 0 && oy == 0 && oz == 0) continue;
+        long long cj = c + oz * L.sz() + oy * L.sy() + ox;
+        T uj = PS[cj + fs], vj = PS[cj + 2 * fs], wj = PS[cj + 3 * fs];
+        T dx = -(T)ox * P.h + xix - hdt * (PR[cj + fs] + uj);
+        T dy = -(T)oy * P.h + xiy - hdt * (PR[cj + 2 * fs] + vj);
+        T dz = -(T)oz * P.h + xiz - hdt * (PR[cj + 3 * fs] + wj);
+        T r2 = dx * dx + dy * dy + dz * dz;
+        T qq = sqrt(r2) * P.inv_h;
+        T pw = PS[cj] * spline_g<T>(qq);
+        sx += pw * dx; sy += pw * dy; sz += pw * dz;
+        se += pw * ((ui + uj) * dx + (vi + vj) * dy + (wi + wj) * dz);
+      }
+  T rho = U[c];
+  T fx = F[c], fy = F[c + fs], fz = F[c + 2 * fs];
+  T pn = phi_i * P.wnorm;
+  T qx = pn * sx + rho * fx;
+  T qy = pn * sy + rho * fy;
+  T qz = pn * sz + rho * fz;
+  T qe = (T)0.5 * pn * se + rho * ((ui * fx + vi * fy) + wi * fz);
+  T mx = (T)0.5 * (U[c + fs] + US[c]) + hdt * qx;
+  T my = (T)0.5 * (U[c + 2 * fs] + US[c + fs]) + hdt * qy;
+  T mz = (T)0.5 * (U[c + 3 * fs] + US[c + 2 * fs]) + hdt * qz;
+  T E = (T)0.5 * (U[c + 4 * fs] + US[c + 3 * fs]) + hdt * qe;
+  UT[c] = mx; UT[c + fs] = my; UT[c + 2 * fs] = mz; UT[c + 3 * fs] = E;
+  T ir = rho > P.rho_vac ? (T)1 / rho : (T)0;
+  T qdt = (T)0.25 * dt;
+  XI[c] = (T)0.5 * xix + qdt * (un + mx * ir);
+  XI[c + fs] = (T)0.5 * xiy + qdt * (vn + my * ir);
+  XI[c + 2 * fs] = (T)0.5 * xiz + qdt * (wn + mz * ir);
+}
+
+template <class T>
+__device__ __forceinline__ T minmod(T a, T b) {
+  if (a > (T)0 && b > (T)0) return a < b ? a : b;
+  if (a < (T)0 && b < (T)0) return a > b ? a : b;
+  return (T)0;
+}
+
+// O7: one face flux, Eq. (8) + pressureless HLL (G10-G13).  cL/cR: cells left/right of the
+// face along axis d (stride sd); returns F[5].
+template <class T>
+__device__ __forceinline__ void face_flux(const Params<T>& P, const T* __restrict__ U, const T* __restrict__ UT,
+                                          const T* __restrict__ XI, long long cL, long long sd, int d, T* Fl) {
+  const long long fs = P.L.fstride;
+  long long cR = cL + sd;
+  T UL[5], UR[5];
+  T xL = XI[cL + d * fs], xR = XI[cR + d * fs];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    const T* Uq = U + q * fs;
+    T a = Uq[cL - sd], b = Uq[cL], c = Uq[cR], e = Uq[cR + sd];
+    T thL = minmod<T>((b - a) * P.inv_h, (c - b) * P.inv_h);
+    T thR = minmod<T>((c - b) * P.inv_h, (e - c) * P.inv_h);
+    T tL = q == 0 ? b : UT[cL + (q - 1) * fs];       // rho~ = rho^n (G2)
+    T tR = q == 0 ? c : UT[cR + (q - 1) * fs];
+    T hL = (T)0.5 * (b + tL), hR = (T)0.5 * (c + tR);  // U^{n+1/2} (G10)
+    UL[q] = hL + (T)0.5 * (P.h - xL) * thL;
+    UR[q] = hR - (T)0.5 * (P.h + xR) * thR;
+  }
+  T uL = UL[0] > P.rho_vac ? UL[1 + d] / UL[0] : (T)0;
+  T uR = UR[0] > P.rho_vac ? UR[1 + d] / UR[0] : (T)0;
+  T up = uL > (T)0 ? uL : (T)0, um = uR < (T)0 ? uR : (T)0;
+#pragma unroll
+  for (int q = 0; q < 5; ++q) Fl[q] = up * UL[q] + um * UR[q];
+}
+
+// O7+O8: FGC + SUE, Eq. (4) unsplit (G14), interior cells; epilogue: CFL speed of U^{n+1}.
+template <class T>
+__global__ void k_euler(Params<T> P, const DevScalars<T>* sc, const T* __restrict__ U, const T* __restrict__ UT,
+                        const T* __restrict__ XI, T* __restrict__ UN, typename Real<T>::bits_t* smax_out) {
+  const Layout& L = P.L;
+  long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  int i, j, k;
+  T s = 0;
+  if (decode_ext(L, 0, m, i, j, k)) {
+    T dt = load_dt(sc);
+    long long c = L.idx(i, j, k), fs = L.fstride;
+    T acc[5] = {0, 0, 0, 0, 0};
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      long long sd = d == 0 ? 1 : (d == 1 ? L.sy() : L.sz());
+      T Fp[5], Fm[5];
+      face_flux<T>(P, U, UT, XI, c, sd, d, Fp);
+      face_flux<T>(P, U, UT, XI, c - sd, sd, d, Fm);
+#pragma unroll
+      for (int q = 0; q < 5; ++q) acc[q] += Fp[q] - Fm[q];
+    }
+    T lam = dt * P.inv_h;
+    T un[5];
+    un[0] = U[c] - lam * acc[0];
+#pragma unroll
+    for (int q = 1; q < 5; ++q) un[q] = UT[c + (q - 1) * fs] - lam * acc[q];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) UN[c + q * fs] = un[q];
+    s = cell_speed_exact<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
+  }
+  block_max_to_global<T>(s, smax_out);
+}
+
+}  // namespace cspt

@@ -1,0 +1,224 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by
+element, on the same seeded inputs.  Tolerances (BASELINE.json north_star; DESIGN.md
+section 6): fp64 1e-11 normwise per conserved field after 10 steps, fp32 1e-4 against
+the fp64 oracle started from the fp32-rounded inputs with the same dt sequence (G22);
+CFL dt and vacuum mask bit-exact on the same input state.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle_util import make_oracle, run_to
+from paper_1912_04855_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-11
+TOL32 = 1e-4
+
+
+@pytest.fixture(scope="module")
+def cspt():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1912_04855_b200 import build, cspt as mod
+    build.build()
+    mod.lib()          # fails loudly if libcspt.so is missing
+    return mod
+
+
+def make_solver(cspt, w, dtype=None):
+    d = cspt.F64 if (dtype or w.dtype) == "f64" else cspt.F32
+    return cspt.Solver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, d)
+
+
+def field_errors(gpu, orc):
+    """Normwise max error per conserved field (G21).  A momentum component that vanishes
+    identically in the oracle is measured against the momentum scale sqrt(rho E)."""
+    gpu = [np.asarray(a, dtype=np.float64) for a in gpu]
+    orc = [np.asarray(a, dtype=np.float64) for a in orc]
+    mscale = math.sqrt(float(np.max(np.abs(orc[0]))) * float(np.max(np.abs(orc[4]))))
+    errs = []
+    for q in range(5):
+        den = float(np.max(np.abs(orc[q])))
+        if 1 <= q <= 3 and den < 1e-6 * mscale:
+            den = mscale
+        errs.append(float(np.max(np.abs(gpu[q] - orc[q]))) / max(den, 1e-300))
+    return errs
+
+
+def run_pair(cspt, orc_mod, w, steps, tol, gpu_dtype=None, fields=None, check_dt=True):
+    """Steps both sides with the oracle's dt sequence; returns (solver, oracle)."""
+    f = fields if fields is not None else w.fields()
+    gd = gpu_dtype or w.dtype
+    o = make_oracle(orc_mod, w, dtype="f64" if gd == "f32" else w.dtype)
+    o.set_state(*[np.asarray(a, dtype=np.float64) for a in f] if gd == "f32" else f)
+    s = make_solver(cspt, w, dtype=gd)
+    s.set_state(*f)
+    if check_dt and gd == "f64":
+        assert s.compute_dt(w.cfl) == o.compute_dt(w.cfl)          # bit-exact on the same input
+    for n in range(steps):
+        dt = o.compute_dt(w.cfl)
+        if gd == "f32":
+            dt = float(np.float32(dt))
+        o.step(dt)
+        s.step(dt)
+    got = [t.cpu().numpy() for t in s.get_conserved()]
+    errs = field_errors(got, o.get_conserved())
+    assert all(np.isfinite(a).all() for a in got)
+    assert max(errs) < tol, errs
+    return s, o
+
+
+# ---- element-by-element, several tiles and a ragged tail, every boundary kind -----------------
+@pytest.mark.parametrize("dims,bc", [
+    ((40, 37, 21), [0] * 6),
+    ((33, 18, 45), [1] * 6),
+    ((24, 20, 19), [2, 1, 0, 0, 1, 1]),
+    ((17, 5, 4), [1, 2, 2, 1, 0, 0]),
+    ((5, 1, 3), [0] * 6),
+])
+def test_random_smooth_fp64(cspt, oracle_mod, dims, bc):
+    w = wl.random_smooth(*dims, bc=bc)
+    run_pair(cspt, oracle_mod, w, 10, TOL64)
+
+
+def test_random_smooth_fp32(cspt, oracle_mod):
+    w = wl.random_smooth(40, 37, 21, dtype="f32")
+    run_pair(cspt, oracle_mod, w, 10, TOL32)
+    # and the fp32 GPU path against the fp32 oracle instance: same arithmetic type
+    o32 = make_oracle(oracle_mod, w)
+    s = make_solver(cspt, w)
+    f = w.fields()
+    o32.set_state(*f)
+    s.set_state(*f)
+    assert np.float32(s.compute_dt(w.cfl)) == np.float32(o32.compute_dt(w.cfl))     # bit-exact in fp32 too
+
+
+# ---- the five BASELINE.json configs at sizes the oracle finishes in seconds ------------------------
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_cfg1_sod(cspt, oracle_mod, axis):
+    w = wl.sod(axis=axis)
+    run_pair(cspt, oracle_mod, w, 10, TOL64)
+
+
+def test_cfg1_sod_full_run_vs_exact(cspt, oracle_mod):
+    """The whole config-1 run with the GPU's own compute_dt: 70 steps to t = 0.2, compared with the
+    exact Riemann solution to the same L1 bound the oracle is pinned to."""
+    import exact_riemann as er
+    w = wl.sod()
+    s = make_solver(cspt, w)
+    s.set_state(*w.fields())
+    t, n = 0.0, 0
+    while t < w.t_end * (1 - 1e-14):
+        dt = min(s.compute_dt(w.cfl), w.t_end - t)
+        s.step(dt)
+        t += dt
+        n += 1
+    rho = s.get_state()[0].cpu().numpy()[0, 0, :]
+    x = (np.arange(w.nx) + 0.5) / w.nx
+    re, _, _ = er.sample((x - 0.5) / w.t_end, 1.0, 0.0, 1.0, 0.125, 0.0, 0.1, 1.4)
+    assert n == 70
+    assert float(np.mean(np.abs(rho - re))) < 1.3e-2
+    o = make_oracle(oracle_mod, w)
+    o.set_state(*w.fields())
+    run_to(o, w.cfl, t_end=w.t_end)
+    assert np.max(np.abs(rho - o.get_state()[0][0, 0, :])) < 1e-9       # 70 steps through a shock
+
+
+def test_cfg2_sedov(cspt, oracle_mod):
+    run_pair(cspt, oracle_mod, wl.sedov(n=28), 10, TOL64)
+
+
+@pytest.mark.parametrize("variant", ["flow", "gamma2", "isothermal"])
+def test_cfg3_well(cspt, oracle_mod, variant):
+    w = wl.well(n=28, variant=variant)
+    s, o = run_pair(cspt, oracle_mod, w, 10, TOL64)
+    if variant == "gamma2":      # well-balanced: the GPU path keeps the exact discrete equilibrium too
+        rho, u, v, ww, p = [t.cpu().numpy() for t in s.get_state()]
+        assert max(np.max(np.abs(a)) for a in (u, v, ww)) < 1e-13
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_cfg4_turbulence(cspt, oracle_mod, dtype):
+    w = wl.turbulence(n=32, dtype=dtype)
+    run_pair(cspt, oracle_mod, w, 10, TOL64 if dtype == "f64" else TOL32)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_cfg5_disk_vacuum(cspt, oracle_mod, dtype):
+    w = wl.disk(n=40, dtype=dtype)
+    s, o = run_pair(cspt, oracle_mod, w, 10, TOL64 if dtype == "f64" else TOL32)
+    # vacuum mask: bit-exact on the same state (push the oracle's state through the GPU getters)
+    o_state = o.get_conserved()
+    s.set_conserved(*[a.astype(np.float32 if dtype == "f32" else np.float64) for a in o_state])
+    if dtype == "f64":
+        assert np.array_equal(s.get_vacuum_mask().cpu().numpy(), o.get_vacuum_mask())
+        assert s.compute_dt(w.cfl) == o.compute_dt(w.cfl)
+        for a, b in zip(s.get_state(), o.get_state()):
+            assert np.array_equal(a.cpu().numpy(), b)            # primitives use exactly rounded operations
+    m = s.get_vacuum_mask().cpu().numpy()
+    assert 0 < m.sum() < m.size                                  # the case really has gas and vacuum
+
+
+# ---- degenerate cases ---------------------------------------------------------------------------
+def test_all_vacuum_grid(cspt, oracle_mod):
+    import torch
+    z = np.zeros((4, 4, 8))
+    s = cspt.Solver(8, 4, 4, 0.1, 1.4, [1] * 6)
+    s.set_state(z, z, z, z, z, z)
+    assert s.compute_dt(0.4) == float("inf")
+    assert s.get_vacuum_mask().min().item() == 1
+    s.step_cfl(0.4)              # dt = +inf on the device: identity step, no NaN
+    assert all(torch.equal(t, torch.zeros_like(t)) for t in s.get_conserved())
+
+
+def test_single_cell_and_thin_grids(cspt, oracle_mod):
+    for dims in [(1, 1, 1), (2, 1, 1), (1, 7, 1)]:
+        w = wl.random_smooth(*dims)
+        run_pair(cspt, oracle_mod, w, 3, TOL64)
+
+
+def test_step_cfl_matches_compute_dt_then_step(cspt, oracle_mod):
+    import torch
+    w = wl.random_smooth(20, 12, 9)
+    a, b = make_solver(cspt, w), make_solver(cspt, w)
+    a.set_state(*w.fields())
+    b.set_state(*w.fields())
+    for _ in range(4):
+        dt = a.compute_dt(w.cfl)
+        a.step(dt)
+        assert b.step_cfl(w.cfl, want_dt=True) == dt
+    for x, y in zip(a.get_conserved(), b.get_conserved()):
+        assert torch.equal(x, y)
+
+
+def test_host_entry_points_roundtrip(cspt, oracle_mod):
+    import torch
+    w = wl.random_smooth(20, 12, 9)
+    f = [torch.from_numpy(a).pin_memory() for a in w.fields()]
+    a, b = make_solver(cspt, w), make_solver(cspt, w)
+    a.set_state(*w.fields())
+    b.set_state_host(*f)
+    a.step(1e-3)
+    b.step(1e-3)
+    out = [torch.empty(a.shape, dtype=torch.float64).pin_memory() for _ in range(5)]
+    b.get_conserved_host(out)
+    for x, y in zip(a.get_conserved(), out):
+        assert torch.equal(x.cpu(), y)
+
+
+def test_errors(cspt):
+    s = cspt.Solver(8, 8, 8, 0.1, 1.4, [0] * 6)
+    with pytest.raises(cspt.CsptError) as e:
+        s.step(0.1)
+    assert e.value.code == cspt.ESTATE
+    z = np.ones((8, 8, 8))
+    s.set_state(z, 0 * z, 0 * z, 0 * z, z, 0 * z)
+    for bad in (0.0, -1.0, float("nan"), float("inf")):
+        with pytest.raises(cspt.CsptError) as e:
+            s.step(bad)
+        assert e.value.code == cspt.EINVAL
+    with pytest.raises(cspt.CsptError):
+        s.compute_dt(0.0)
