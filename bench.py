@@ -1,0 +1,380 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the CSPH-TVD step (BASELINE.json metric) on N B200s.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cspt|reference]
+                    [--workload turbulence|sedov|well|disk|sod] [--n SIZE] [--dtype f64|f32]
+
+A "step" is one pass of the whole hot path over the grid: CFL time step (device
+resident), ghost fill, Lagrangian predictor/corrector, Eulerian flux + update
+(`cspt_step_cfl`).  The default workload is BASELINE.json configs[3], the 512^3 fp64
+smooth periodic field the north_star target is quoted on.  Prints ONE JSON line
+(rank 0).  N > 1: the path does not shard (north_star: one GPU, no collectives;
+DESIGN.md section 8) so N independent replicas run, one per GPU ("replicas only").
+
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of
+the same workload on the host cores; it is the only leg besides `cpu_baseline` that
+executes oracle/.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "Mcell-updates/s per CSPH-TVD step"
+UNIT = "Mcell-updates/s"
+# SURVEY.md 8(d) / DESIGN.md section 7: minimum HBM traffic of one cell-update = read
+# 5 conserved fields + psi, write 5 conserved fields = 11 words.
+MIN_WORDS_PER_CELL = 11
+
+# Algorithmic words per cell of each kernel of the step ("kernels"):
+# the fields a kernel must read once and write once, nothing for stencil re-reads.
+KERNEL_WORDS = {
+    "prim": 5 + 4,                 # U^n -> phi,u,v,w
+    "predictor": 4 + 5 + 3 + 8,    # prim, U^n, f -> U*, prim*
+    "corrector": 4 + 5 + 3 + 8 + 7,  # prim, U^n, f, U*, prim* -> U~, xi
+    "euler": 5 + 4 + 3 + 5,        # U^n, U~, xi -> U^{n+1}
+    "lagrange": 5 + 3 + 7,         # fused predictor+corrector: U^n, f -> U~, xi
+    "step_fused": 5 + 3 + 5,       # fully fused step: U^n, f -> U^{n+1}
+    "speed_max": 5,
+}
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cspt", choices=["cspt", "reference"])
+    ap.add_argument("--workload", default="turbulence")
+    ap.add_argument("--n", type=int, default=None, help="grid size override (default: the config's)")
+    ap.add_argument("--dtype", default=None, choices=["f64", "f32"])
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def peaks():
+    """Measured roofline denominators (driver-written), else the profiling guide's fallback."""
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as fh:
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md, 6.65 TB/s)"
+
+
+# ---------------------------------------------------------------------------------------
+# clocks: NVML samples DURING the timed region
+# ---------------------------------------------------------------------------------------
+_REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+            0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+
+class ClockSampler:
+    def __init__(self, device_index):
+        self.samples, self.mask, self.ok = [], 0, False
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            h = None
+            try:
+                uuid = str(torch.cuda.get_device_properties(device_index).uuid)
+                if not uuid.startswith("GPU-"):
+                    uuid = "GPU-" + uuid
+                h = pynvml.nvmlDeviceGetHandleByUUID(uuid.encode() if hasattr(uuid, "encode") else uuid)
+            except Exception:
+                vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+                idx = device_index
+                if vis:
+                    try:
+                        idx = int(vis.split(",")[device_index])
+                    except Exception:
+                        idx = device_index
+                h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.h = h
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception as e:  # no NVML: report that, never fake a clock
+            self.err = repr(e)
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    self.mask |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                except Exception:
+                    self.mask |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+            except Exception:
+                pass
+            self._stop.wait(0.02)
+
+    def start(self):
+        if self.ok:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        if self._thr:
+            self._stop.set()
+            self._thr.join()
+        if not self.ok or not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable"]}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "samples": len(s),
+                "reasons": [name for bit, name in sorted(_REASONS.items()) if self.mask & bit]}
+
+
+# ---------------------------------------------------------------------------------------
+# workload
+# ---------------------------------------------------------------------------------------
+def make_workload(args):
+    from paper_1912_04855_b200 import workloads as wl
+    w = wl.by_name(args.workload, n=args.n, dtype=args.dtype)
+    return w
+
+
+def config_of(w, world):
+    esz = 8 if w.dtype == "f64" else 4
+    name = "%s %dx%dx%d %s" % (w.name, w.nx, w.ny, w.nz, w.dtype)
+    if w.name == "turbulence":
+        name += " (BASELINE.json configs[3])"
+    big = 5 * w.cells * esz > 4 * 126e6
+    return {"workload": name, "cfl": w.cfl, "gamma": w.gamma, "bc": list(w.bc),
+            "parallelism": "replicas only" if world > 1 else "1 gpu",
+            "l2": ("state (%.1f GiB) larger than L2, no flush needed" % (5 * w.cells * esz / 2 ** 30)) if big
+            else "state fits L2: measures launch latency / L2, not HBM"}
+
+
+def host_fields(w, pin):
+    """The six input fields as (pinned) host tensors, generated slab by slab on a few threads."""
+    import numpy as np
+    import torch
+    from concurrent.futures import ThreadPoolExecutor
+    tdt = torch.float64 if w.dtype == "f64" else torch.float32
+    out = [torch.empty((w.nz, w.ny, w.nx), dtype=tdt) for _ in range(6)]
+    if pin:
+        out = [t.pin_memory() for t in out]
+    views = [t.numpy() for t in out]
+    slab = max(1, min(w.nz, (1 << 22) // max(1, w.nx * w.ny)))
+
+    def fill(k0):
+        k1 = min(w.nz, k0 + slab)
+        f = w.fields_slab(k0, k1)
+        for v, a in zip(views, f):
+            v[k0:k1] = a
+
+    with ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1)) as ex:
+        list(ex.map(fill, range(0, w.nz, slab)))
+    return out
+
+
+# ---------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline and --impl reference)
+# ---------------------------------------------------------------------------------------
+def oracle_sample(args, w_full, steps, warmup, n_sample):
+    """Times `steps` oracle steps (compute_dt + step) on an n_sample^3 instance of the
+    workload, all host cores (bit-identical for any thread count).  Returns per-step seconds."""
+    from oracle import csph_oracle as orc
+    from paper_1912_04855_b200 import workloads as wl
+    cores = os.cpu_count() or 1
+    try:
+        cores = len(os.sched_getaffinity(0))
+    except Exception:
+        pass
+    orc.build()
+    orc.set_threads(cores)
+    w = wl.by_name(args.workload, n=n_sample, dtype=w_full.dtype)
+    o = orc.Oracle(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, orc.F64 if w.dtype == "f64" else orc.F32)
+    o.set_state(*w.fields())
+    for _ in range(warmup):
+        o.step(o.compute_dt(w.cfl))
+    times = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        o.step(o.compute_dt(w.cfl))
+        times.append(time.perf_counter() - t0)
+    o.close()
+    return w, times, cores
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w_full = make_workload(args)
+    # bounded sample: a 96^3 instance (64^3 for long runs) so the whole run ends within minutes
+    n_s = min(96 if (args.steps + args.warmup) <= 60 else 64, max(w_full.nx, w_full.ny, w_full.nz))
+    if args.workload == "sod":
+        n_s = None
+    w, times, cores = oracle_sample(args, w_full, args.steps, args.warmup, n_s)
+    tot = sum(times)
+    val = w.cells * len(times) / tot / 1e6
+    sample = ("each step = one oracle step (compute_dt + step) on a %dx%dx%d instance of the workload (%s), %d threads"
+              % (w.nx, w.ny, w.nz, w.dtype, cores))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": w.dtype, "data": "synthetic",
+        "config": config_of(w_full, max(1, args.gpus)),
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------
+# the CUDA path
+# ---------------------------------------------------------------------------------------
+def run_cspt(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1912_04855_b200 import build, cspt
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the CSPH-TVD path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    cspt.lib()
+
+    w = make_workload(args)
+    esz = 8 if w.dtype == "f64" else 4
+    dtype = cspt.F64 if w.dtype == "f64" else cspt.F32
+    fields = host_fields(w, pin=True)
+    s = cspt.Solver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, dtype)
+    s.set_state_host(*fields)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        s.step_cfl(w.cfl)
+    barrier()
+
+    # ---- timed region: exactly K steps, device time from CUDA events on the launching stream
+    sampler = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = s.launch_count()
+    s.profile_enable(True)
+    sampler.start()
+    e0.record(s.stream)
+    for _ in range(args.steps):
+        s.step_cfl(w.cfl)
+    e1.record(s.stream)
+    barrier()
+    clocks = sampler.stop()
+    ms = e0.elapsed_time(e1)
+    prof = s.profile_read()
+    s.profile_enable(False)
+    launches = s.launch_count() - l0
+    tmax = ms
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        tmax = float(t.item())
+    value = world * w.cells * args.steps / (tmax * 1e-3) / 1e6
+
+    # the state must still be sane (a blown-up run would time NaN arithmetic)
+    rho = s.get_conserved()[0]
+    assert bool(torch.isfinite(rho).all()), "state is not finite after the timed steps"
+
+    # ---- end to end through the C ABI with HOST buffers: H2D of the 6 inputs, one step, D2H of U
+    out = [torch.empty((w.nz, w.ny, w.nx), dtype=fields[0].dtype).pin_memory() for _ in range(5)]
+    n_e2e = max(1, args.e2e_steps)
+    s.set_state_host(*fields)
+    s.step_cfl(w.cfl)
+    s.get_conserved_host(out)           # warm-up of the host path
+    barrier()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record(s.stream)
+    for _ in range(n_e2e):
+        s.set_state_host(*fields)
+        s.step_cfl(w.cfl)
+        s.get_conserved_host(out)
+    f1.record(s.stream)
+    barrier()
+    ems = f0.elapsed_time(f1)
+    if world > 1:
+        t = torch.tensor([ems], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ems = float(t.item())
+    e2e = {"value": world * w.cells * n_e2e / (ems * 1e-3) / 1e6, "unit": UNIT,
+           "h2d_bytes_per_step": 6 * w.cells * esz, "d2h_bytes_per_step": 5 * w.cells * esz, "steps": n_e2e,
+           "what": "cspt_set_state_host + cspt_step_cfl + cspt_get_conserved_host per step, pinned host buffers"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel, from the event pairs recorded in the timed region
+    peak, peak_src = peaks()
+    step_ms = tmax / args.steps
+    kern = {k: {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps} for k, v in prof.items()}
+    dom = max(prof.items(), key=lambda kv: kv[1][0])[0]
+    dom_ms = prof[dom][0] / prof[dom][1]
+    words = KERNEL_WORDS.get(dom, MIN_WORDS_PER_CELL)
+    dom_bytes = words * esz * w.cells
+    ach = dom_bytes / (dom_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": dom_bytes,
+                "kernel_ms": dom_ms, "share_of_step": (prof[dom][0] / args.steps) / step_ms}
+    step_ach = MIN_WORDS_PER_CELL * esz * w.cells / (step_ms * 1e-3) / 1e9
+    step_hbm = {"bytes_per_cell_update": MIN_WORDS_PER_CELL * esz, "achieved_gbs": step_ach, "frac_of_measured": step_ach / peak,
+                "frac_of_nominal_8TBs": step_ach / 8000.0}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": w.dtype, "data": "synthetic",
+        "config": config_of(w, world),
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "kernels": kern,
+        "roofline": roofline, "step_hbm": step_hbm,
+    }
+
+    if not args.no_cpu_baseline and world == 1:
+        n_s = min(160, max(w.nx, w.ny, w.nz)) if args.workload != "sod" else None
+        ws, times, cores = oracle_sample(args, w, 3, 0, n_s)
+        tot = sum(times)
+        line["cpu_baseline"] = {"value": ws.cells * len(times) / tot / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": "%s instance %dx%dx%d (%s), 3 steps (compute_dt + step), %d threads; %.1f s"
+                                % (ws.name, ws.nx, ws.ny, ws.nz, ws.dtype, cores, tot)}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cspt(args)
+
+
+if __name__ == "__main__":
+    main()

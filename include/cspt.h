@@ -95,6 +95,15 @@ int cspt_get_vacuum_mask(cspt_ctx*, unsigned char* mask);
 
 /* Number of kernel launches issued by this ctx so far (for bench.py's gpu_launches). */
 long long cspt_launch_count(const cspt_ctx*);
+/* Per-kernel device timing.  While enabled, every kernel the ctx launches is bracketed
+ * by a CUDA event pair on the ctx's stream (up to 8192 launches since the last enable;
+ * later ones are not recorded).  on != 0 resets the record.  cspt_profile_read sums the
+ * device time and counts the launches of kernel `kid` (0 <= kid < cspt_profile_kernel_count(),
+ * named by cspt_profile_kernel_name); it syncs.  Used by bench.py for the roofline figure. */
+int cspt_profile_enable(cspt_ctx*, int on);
+int cspt_profile_kernel_count(void);
+const char* cspt_profile_kernel_name(int kid);
+int cspt_profile_read(cspt_ctx*, int kid, double* total_ms, long long* launches);
 /* Waits for the ctx's stream. */
 int cspt_sync(cspt_ctx*);
 /* Frees the ctx, never the workspace.  NULL is allowed. */

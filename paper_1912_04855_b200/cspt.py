@@ -30,6 +30,10 @@ SYMBOLS = [
     ("cspt_set_conserved", _ci, [_vp] * 6),
     ("cspt_get_vacuum_mask", _ci, [_vp, _vp]),
     ("cspt_launch_count", ctypes.c_longlong, [_vp]),
+    ("cspt_profile_enable", _ci, [_vp, _ci]),
+    ("cspt_profile_kernel_count", _ci, []),
+    ("cspt_profile_kernel_name", ctypes.c_char_p, [_ci]),
+    ("cspt_profile_read", _ci, [_vp, _ci, _pd, ctypes.POINTER(ctypes.c_longlong)]),
     ("cspt_sync", _ci, [_vp]),
     ("cspt_destroy", None, [_vp]),
     ("cspt_strerror", ctypes.c_char_p, [_ci]),
@@ -177,6 +181,20 @@ class Solver:
 
     def launch_count(self):
         return int(lib().cspt_launch_count(self._h))
+
+    def profile_enable(self, on=True):
+        _check(lib().cspt_profile_enable(self._h, 1 if on else 0), "cspt_profile_enable")
+
+    def profile_read(self):
+        """{kernel name: (total device ms, launches)} since profile_enable(True)."""
+        L = lib()
+        out = {}
+        for kid in range(L.cspt_profile_kernel_count()):
+            ms, n = ctypes.c_double(), ctypes.c_longlong()
+            _check(L.cspt_profile_read(self._h, kid, ctypes.byref(ms), ctypes.byref(n)), "cspt_profile_read")
+            if n.value:
+                out[L.cspt_profile_kernel_name(kid).decode()] = (ms.value, int(n.value))
+        return out
 
     def sync(self):
         _check(lib().cspt_sync(self._h), "cspt_sync")

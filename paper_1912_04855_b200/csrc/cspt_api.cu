@@ -66,9 +66,26 @@ inline int blocks_for(long long n, int threads, int cap = 0) {
 constexpr int TPB = 256;
 constexpr int STRIDE_CAP = 148 * 16;   // grid-stride kernels: 16 CTAs of 256 threads per SM
 
-#define LAUNCH(ctx, kernel, grid, block, ...)                     \
+// Event pair around one launch when cspt_profile_enable is on (device time per kernel).
+const char* const kKernelNames[K_COUNT] = {"ghost_fill", "prim", "predictor", "corrector", "euler", "speed_max",
+                                           "scalar", "io", "force"};
+
+inline int prof_open(cspt_ctx* c, int kid) {
+  if (!c->prof_on || c->prof_used >= c->prof_cap) return -1;
+  int s = c->prof_used++;
+  c->prof_kid[s] = kid;
+  cudaEventRecord(c->prof_ev[2 * s], c->stream);
+  return s;
+}
+inline void prof_close(cspt_ctx* c, int s) {
+  if (s >= 0) cudaEventRecord(c->prof_ev[2 * s + 1], c->stream);
+}
+
+#define LAUNCH(ctx, kid, kernel, grid, block, ...)                \
   do {                                                            \
+    int ps_ = prof_open((ctx), (kid));                            \
     kernel<<<(grid), (block), 0, (ctx)->stream>>>(__VA_ARGS__);   \
+    prof_close((ctx), ps_);                                       \
     (ctx)->launches++;                                            \
   } while (0)
 
@@ -93,7 +110,7 @@ void fill_ghosts(cspt_ctx* c, T* F, int nfields, int mode) {
     int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
     long long e1 = d1 < d ? n[d1] + 2 * NG : n[d1], e2 = d2 < d ? n[d2] + 2 * NG : n[d2];
     long long total = e1 * e2 * NG * 2;
-    LAUNCH(c, k_ghost_axis<T>, blocks_for(total, TPB, STRIDE_CAP), TPB, L, d, mode, c->bc[2 * d], c->bc[2 * d + 1],
+    LAUNCH(c, K_GHOST, k_ghost_axis<T>, blocks_for(total, TPB, STRIDE_CAP), TPB, L, d, mode, c->bc[2 * d], c->bc[2 * d + 1],
            nfields, F, inflow<T>(c, 2 * d), inflow<T>(c, 2 * d + 1), c->inflow_plane);
   }
 }
@@ -104,11 +121,11 @@ int set_state_t(cspt_ctx* c, const void* rho, const void* u, const void* v, cons
   long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
   T* U = field<T>(c, S_U0);
   T* psi_pad = field<T>(c, S_UT);          // scratch: U~ is dead between steps
-  LAUNCH(c, k_set_state<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, (const T*)rho, (const T*)u, (const T*)v,
+  LAUNCH(c, K_IO, k_set_state<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, (const T*)rho, (const T*)u, (const T*)v,
          (const T*)w, (const T*)p, (const T*)psi, U, psi_pad);
   fill_ghosts<T>(c, psi_pad, 1, 2);
   long long ne = (long long)(c->L.nx + 4) * (c->L.ny + 4) * (c->L.nz + 4);
-  LAUNCH(c, k_force<T>, blocks_for(ne, TPB, STRIDE_CAP), TPB, P, psi_pad, field<T>(c, S_F));
+  LAUNCH(c, K_FORCE, k_force<T>, blocks_for(ne, TPB, STRIDE_CAP), TPB, P, psi_pad, field<T>(c, S_F));
   fill_ghosts<T>(c, U, 5, 1);
   c->cur = 0;
   c->has_state = true;
@@ -121,7 +138,7 @@ int set_conserved_t(cspt_ctx* c, const void* const in[5]) {
   long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
   T* U = field<T>(c, c->cur ? S_U1 : S_U0);
   for (int f = 0; f < 5; ++f)
-    LAUNCH(c, k_put_field<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, c->L, (const T*)in[f], U + f * c->L.fstride);
+    LAUNCH(c, K_IO, k_put_field<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, c->L, (const T*)in[f], U + f * c->L.fstride);
   c->smax_valid = false;
   return check(c);
 }
@@ -131,7 +148,7 @@ int get_conserved_t(cspt_ctx* c, void* const out[5]) {
   long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
   const T* U = field<T>(c, c->cur ? S_U1 : S_U0);
   for (int f = 0; f < 5; ++f)
-    LAUNCH(c, k_get_field<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, c->L, U + f * c->L.fstride, (T*)out[f]);
+    LAUNCH(c, K_IO, k_get_field<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, c->L, U + f * c->L.fstride, (T*)out[f]);
   return check(c);
 }
 
@@ -140,7 +157,7 @@ int get_state_t(cspt_ctx* c, void* rho, void* u, void* v, void* w, void* p, unsi
   Params<T> P = make_params<T>(c);
   long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
   const T* U = field<T>(c, c->cur ? S_U1 : S_U0);
-  LAUNCH(c, k_get_state<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, U, (T*)rho, (T*)u, (T*)v, (T*)w, (T*)p, mask);
+  LAUNCH(c, K_IO, k_get_state<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, U, (T*)rho, (T*)u, (T*)v, (T*)w, (T*)p, mask);
   return check(c);
 }
 
@@ -149,8 +166,8 @@ void ensure_smax(cspt_ctx* c) {
   if (c->smax_valid) return;
   Params<T> P = make_params<T>(c);
   long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
-  LAUNCH(c, k_reset_smax<T>, 1, 1, scalars<T>(c));
-  LAUNCH(c, k_speed_max<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, field<T>(c, c->cur ? S_U1 : S_U0),
+  LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, scalars<T>(c));
+  LAUNCH(c, K_SPEED_MAX, k_speed_max<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, field<T>(c, c->cur ? S_U1 : S_U0),
          &scalars<T>(c)->smax_bits);
   c->smax_valid = true;
 }
@@ -187,13 +204,13 @@ void run_step(cspt_ctx* c) {
   long long n2 = (long long)(L.nx + 4) * (L.ny + 4) * (L.nz + 4);
   long long n1 = (long long)(L.nx + 2) * (L.ny + 2) * (L.nz + 2);
   long long n0 = (long long)L.nx * L.ny * L.nz;
-  LAUNCH(c, k_prim<T>, blocks_for(n3, TPB), TPB, P, U, field<T>(c, S_PR));          // O1
-  LAUNCH(c, k_predictor<T>, blocks_for(n2, TPB), TPB, P, sc, U, field<T>(c, S_PR), field<T>(c, S_F),
+  LAUNCH(c, K_PRIM, k_prim<T>, blocks_for(n3, TPB), TPB, P, U, field<T>(c, S_PR));          // O1
+  LAUNCH(c, K_PREDICTOR, k_predictor<T>, blocks_for(n2, TPB), TPB, P, sc, U, field<T>(c, S_PR), field<T>(c, S_F),
          field<T>(c, S_US), field<T>(c, S_PS));                                    // O3, O4
-  LAUNCH(c, k_corrector<T>, blocks_for(n1, TPB), TPB, P, sc, U, field<T>(c, S_PR), field<T>(c, S_F),
+  LAUNCH(c, K_CORRECTOR, k_corrector<T>, blocks_for(n1, TPB), TPB, P, sc, U, field<T>(c, S_PR), field<T>(c, S_F),
          field<T>(c, S_US), field<T>(c, S_PS), field<T>(c, S_UT), field<T>(c, S_XI));   // O5, O6
-  LAUNCH(c, k_reset_smax<T>, 1, 1, sc);
-  LAUNCH(c, k_euler<T>, blocks_for(n0, TPB), TPB, P, sc, U, field<T>(c, S_UT), field<T>(c, S_XI), UN,
+  LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, sc);
+  LAUNCH(c, K_EULER, k_euler<T>, blocks_for(n0, TPB), TPB, P, sc, U, field<T>(c, S_UT), field<T>(c, S_XI), UN,
          &sc->smax_bits);                                                          // O7, O8 (+O9 epilogue)
   c->cur ^= 1;
   c->smax_valid = true;
@@ -201,7 +218,7 @@ void run_step(cspt_ctx* c) {
 
 template <class T>
 int step_t(cspt_ctx* c, double dt) {
-  LAUNCH(c, k_set_dt<T>, 1, 1, scalars<T>(c), (T)dt);
+  LAUNCH(c, K_SCALAR, k_set_dt<T>, 1, 1, scalars<T>(c), (T)dt);
   run_step<T>(c);
   return check(c);
 }
@@ -209,7 +226,7 @@ int step_t(cspt_ctx* c, double dt) {
 template <class T>
 int step_cfl_t(cspt_ctx* c, double cfl, double* out) {
   ensure_smax<T>(c);
-  LAUNCH(c, k_dt_finalize<T>, 1, 1, scalars<T>(c), (T)cfl, (T)c->h);
+  LAUNCH(c, K_SCALAR, k_dt_finalize<T>, 1, 1, scalars<T>(c), (T)cfl, (T)c->h);
   run_step<T>(c);
   int rc = check(c);
   if (rc || !out) return rc;
@@ -275,7 +292,53 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
 void cspt_destroy(cspt_ctx* c) {
   if (!c) return;
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
+  for (int i = 0; i < 2 * c->prof_cap; ++i) cudaEventDestroy(c->prof_ev[i]);
+  delete[] c->prof_ev;
+  delete[] c->prof_kid;
   delete c;
+}
+
+int cspt_profile_enable(cspt_ctx* c, int on) {
+  if (!c) return CSPT_EINVAL;
+  if (c->cuda_error) return CSPT_ECUDA;
+  if (on && !c->prof_ev) {
+    const int cap = 8192;
+    c->prof_ev = new (std::nothrow) cudaEvent_t[2 * cap];
+    c->prof_kid = new (std::nothrow) int[cap];
+    if (!c->prof_ev || !c->prof_kid) { delete[] c->prof_ev; delete[] c->prof_kid; c->prof_ev = nullptr; c->prof_kid = nullptr; return CSPT_ENOMEM; }
+    for (int i = 0; i < 2 * cap; ++i) {
+      int rc = cuda_call(c, cudaEventCreate(&c->prof_ev[i]));
+      if (rc) { c->prof_cap = i / 2; return rc; }
+    }
+    c->prof_cap = cap;
+  }
+  c->prof_on = on != 0;
+  if (on) c->prof_used = 0;
+  return CSPT_OK;
+}
+
+int cspt_profile_kernel_count(void) { return K_COUNT; }
+
+const char* cspt_profile_kernel_name(int kid) { return kid >= 0 && kid < K_COUNT ? kKernelNames[kid] : nullptr; }
+
+int cspt_profile_read(cspt_ctx* c, int kid, double* total_ms, long long* launches) {
+  if (!c || kid < 0 || kid >= K_COUNT || !total_ms || !launches) return CSPT_EINVAL;
+  if (c->cuda_error) return CSPT_ECUDA;
+  int rc = cuda_call(c, cudaStreamSynchronize(c->stream));
+  if (rc) return rc;
+  double ms = 0;
+  long long n = 0;
+  for (int s = 0; s < c->prof_used; ++s) {
+    if (c->prof_kid[s] != kid) continue;
+    float t = 0;
+    rc = cuda_call(c, cudaEventElapsedTime(&t, c->prof_ev[2 * s], c->prof_ev[2 * s + 1]));
+    if (rc) return rc;
+    ms += t;
+    ++n;
+  }
+  *total_ms = ms;
+  *launches = n;
+  return CSPT_OK;
 }
 
 int cspt_set_state(cspt_ctx* c, const void* rho, const void* u, const void* v, const void* w, const void* p,

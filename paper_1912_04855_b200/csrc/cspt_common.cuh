@@ -82,6 +82,9 @@ template <class T> struct DevScalars {
   typename Real<T>::bits_t smax_bits;    // max signal speed, IEEE bits (positive floats order like integers)
 };
 
+// Kernel ids for cspt_profile_* (names in cspt_api.cu, same order).
+enum KernelId { K_GHOST = 0, K_PRIM, K_PREDICTOR, K_CORRECTOR, K_EULER, K_SPEED_MAX, K_SCALAR, K_IO, K_FORCE, K_COUNT };
+
 }  // namespace cspt
 
 struct cspt_ctx {
@@ -102,4 +105,10 @@ struct cspt_ctx {
   // workspace sub-buffers (byte offsets)
   size_t off_fields, off_inflow, off_scalars;
   long long inflow_plane;  // elements per captured plane
+  // per-kernel device timing (cspt_profile_*): event pairs recorded around each launch
+  bool prof_on;
+  int prof_used;                    // pairs recorded since the last reset
+  int prof_cap;                     // pairs allocated
+  cudaEvent_t* prof_ev;             // 2 * prof_cap events
+  int* prof_kid;                    // kernel id of each pair
 };
