@@ -104,6 +104,8 @@ int cspt_profile_enable(cspt_ctx*, int on);
 int cspt_profile_kernel_count(void);
 const char* cspt_profile_kernel_name(int kid);
 int cspt_profile_read(cspt_ctx*, int kid, double* total_ms, long long* launches);
+/* The cudaError_t value behind a CSPT_ECUDA status of this ctx (0 if none). */
+int cspt_cuda_error(const cspt_ctx*);
 /* Waits for the ctx's stream. */
 int cspt_sync(cspt_ctx*);
 /* Frees the ctx, never the workspace.  NULL is allowed. */

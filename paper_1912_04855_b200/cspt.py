@@ -34,6 +34,7 @@ SYMBOLS = [
     ("cspt_profile_kernel_count", _ci, []),
     ("cspt_profile_kernel_name", ctypes.c_char_p, [_ci]),
     ("cspt_profile_read", _ci, [_vp, _ci, _pd, ctypes.POINTER(ctypes.c_longlong)]),
+    ("cspt_cuda_error", _ci, [_vp]),
     ("cspt_sync", _ci, [_vp]),
     ("cspt_destroy", None, [_vp]),
     ("cspt_strerror", ctypes.c_char_p, [_ci]),
@@ -195,6 +196,9 @@ class Solver:
             if n.value:
                 out[L.cspt_profile_kernel_name(kid).decode()] = (ms.value, int(n.value))
         return out
+
+    def cuda_error(self):
+        return int(lib().cspt_cuda_error(self._h))
 
     def sync(self):
         _check(lib().cspt_sync(self._h), "cspt_sync")

@@ -1,9 +1,11 @@
 // cspt_api.cu -- the C ABI declared in include/cspt.h: argument checks, workspace
 // carving and kernel launches.  All arithmetic of the method is in the kernels.
 #include <new>
+#include <stdlib.h>
 #include <string.h>
 
 #include "cspt_step.cuh"
+#include "cspt_euler.cuh"
 
 using namespace cspt;
 
@@ -192,6 +194,48 @@ int compute_dt_t(cspt_ctx* c, double cfl, double* out) {
   return CSPT_OK;
 }
 
+constexpr int ETX = 32, ETY = 8;     // Euler-stage tile (threads = cells of one plane of the column)
+
+int pick_zchunk(int tiles, int nz) {
+  // enough CTAs for ~8 waves of 2 CTAs per SM, but at least 16 planes per CTA (2 extra planes per chunk)
+  int want = (148 * 2 * 8 + tiles - 1) / tiles;
+  int zc = (nz + want - 1) / want;
+  if (zc < 16) zc = 16;
+  if (zc > nz) zc = nz;
+  return zc;
+}
+
+template <class T>
+bool make_maps(cspt_ctx* c) {
+  const Layout& L = c->L;
+  typedef EulerSmem<T, ETX, ETY> S;
+  bool ok = true;
+  for (int b = 0; b < 2; ++b)
+    ok = ok && make_field_map(&c->mapU[b], field<T>(c, b ? S_U1 : S_U0), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 5,
+                              S::BX, S::UY, 5);
+  ok = ok && make_field_map(&c->mapL, field<T>(c, S_UT), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 7, S::BX, S::LY, 7);
+  if (ok) {
+    ok = cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
+         cudaSuccess;
+  }
+  return ok;
+}
+
+template <class T>
+void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
+  typedef EulerSmem<T, ETX, ETY> S;
+  const Layout& L = c->L;
+  int gx = (L.nx + ETX - 1) / ETX, gy = (L.ny + ETY - 1) / ETY;
+  int zc = pick_zchunk(gx * gy, L.nz);
+  dim3 grid(gx, gy, (L.nz + zc - 1) / zc);
+  DevScalars<T>* sc = scalars<T>(c);
+  int ps_ = prof_open(c, K_EULER);
+  k_euler_stream<T, ETX, ETY><<<grid, ETX * ETY, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN,
+                                                                         &sc->smax_bits, zc);
+  prof_close(c, ps_);
+  c->launches++;
+}
+
 template <class T>
 void run_step(cspt_ctx* c) {
   Params<T> P = make_params<T>(c);
@@ -210,8 +254,11 @@ void run_step(cspt_ctx* c) {
   LAUNCH(c, K_CORRECTOR, k_corrector<T>, blocks_for(n1, TPB), TPB, P, sc, U, field<T>(c, S_PR), field<T>(c, S_F),
          field<T>(c, S_US), field<T>(c, S_PS), field<T>(c, S_UT), field<T>(c, S_XI));   // O5, O6
   LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, sc);
-  LAUNCH(c, K_EULER, k_euler<T>, blocks_for(n0, TPB), TPB, P, sc, U, field<T>(c, S_UT), field<T>(c, S_XI), UN,
-         &sc->smax_bits);                                                          // O7, O8 (+O9 epilogue)
+  if (c->legacy_euler)
+    LAUNCH(c, K_EULER, k_euler<T>, blocks_for(n0, TPB), TPB, P, sc, U, field<T>(c, S_UT), field<T>(c, S_XI), UN,
+           &sc->smax_bits);
+  else
+    launch_euler<T>(c, P, U, UN);                                                  // O7, O8 (+O9 epilogue)
   c->cur ^= 1;
   c->smax_valid = true;
 }
@@ -285,6 +332,9 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->stream = (cudaStream_t)cuda_stream;
   carve(c);
   if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
+  c->have_maps = dtype == CSPT_F64 ? make_maps<double>(c) : make_maps<float>(c);
+  if (!c->have_maps) { (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }
+  c->legacy_euler = getenv("CSPT_LEGACY_EULER") != nullptr;
   *out = c;
   return CSPT_OK;
 }
@@ -434,6 +484,8 @@ int cspt_get_vacuum_mask(cspt_ctx* c, unsigned char* mask) {
 }
 
 long long cspt_launch_count(const cspt_ctx* c) { return c ? c->launches : 0; }
+
+int cspt_cuda_error(const cspt_ctx* c) { return c ? c->cuda_error : 0; }
 
 int cspt_sync(cspt_ctx* c) {
   if (!c) return CSPT_EINVAL;

@@ -1,6 +1,7 @@
 // cspt_common.cuh -- grid layout, context and small device helpers of the
 // CUDA CSPH-TVD path (sm_100a).  No code is shared with oracle/.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stddef.h>
@@ -31,8 +32,11 @@ struct Layout {
 inline Layout make_layout(int nx, int ny, int nz) {
   Layout L;
   L.nx = nx; L.ny = ny; L.nz = nz;
+  // minimum extents so that every TMA box of the streaming kernels fits inside the tensor
   L.px = ((nx + GX + NG + 15) / 16) * 16;
+  if (L.px < 64) L.px = 64;
   L.py = ny + 2 * NG;
+  if (L.py < 32) L.py = 32;
   L.pz = nz + 2 * NG;
   long long n = (long long)L.px * L.py * L.pz;
   L.fstride = ((n + 63) / 64) * 64;
@@ -105,6 +109,10 @@ struct cspt_ctx {
   // workspace sub-buffers (byte offsets)
   size_t off_fields, off_inflow, off_scalars;
   long long inflow_plane;  // elements per captured plane
+  // TMA views (x, y, z, field) of the two U buffers and of the (U~, xi) group
+  CUtensorMap mapU[2], mapL;
+  bool have_maps;
+  bool legacy_euler;        // debug switch (env CSPT_LEGACY_EULER): first, unfused Euler kernel
   // per-kernel device timing (cspt_profile_*): event pairs recorded around each launch
   bool prof_on;
   int prof_used;                    // pairs recorded since the last reset
