@@ -6,6 +6,7 @@
 
 #include "cspt_step.cuh"
 #include "cspt_euler.cuh"
+#include "cspt_lagrange.cuh"
 
 using namespace cspt;
 
@@ -195,6 +196,8 @@ int compute_dt_t(cspt_ctx* c, double cfl, double* out) {
 }
 
 constexpr int ETX = 32, ETY = 8;     // Euler-stage tile (threads = cells of one plane of the column)
+// corrector tile: CTX x CTY cells per plane, CCY cells (adjacent in y) per thread, CNST ring stages
+constexpr int CTX = 32, CTY = 8, CCY = 2, CNST = 4;
 
 int pick_zchunk(int tiles, int nz) {
   // enough CTAs for ~8 waves of 2 CTAs per SM, but at least 16 planes per CTA (2 extra planes per chunk)
@@ -218,7 +221,29 @@ bool make_maps(cspt_ctx* c) {
     ok = cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
          cudaSuccess;
   }
+  typedef CorrSmem<T, CTX, CTY, CCY, CNST> SC;
+  ok = ok && make_field_map(&c->mapS, field<T>(c, S_ST), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, SC::NF, SC::BX,
+                            SC::BY, SC::NF);
+  if (ok) {
+    ok = cudaFuncSetAttribute(k_corrector_stream<T, CTX, CTY, CCY, CNST>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              SC::BYTES) == cudaSuccess;
+  }
   return ok;
+}
+
+// HFC/SUL{corrector} over the extended domain interior(+)1
+template <class T>
+void launch_corrector(cspt_ctx* c, const Params<T>& P, const T* U) {
+  typedef CorrSmem<T, CTX, CTY, CCY, CNST> SC;
+  const Layout& L = c->L;
+  int gx = (L.nx + 2 + CTX - 1) / CTX, gy = (L.ny + 2 + CTY - 1) / CTY;
+  int zc = pick_zchunk(gx * gy, L.nz + 2);
+  dim3 grid(gx, gy, (L.nz + 2 + zc - 1) / zc);
+  int ps_ = prof_open(c, K_CORRECTOR);
+  k_corrector_stream<T, CTX, CTY, CCY, CNST><<<grid, SC::THREADS, SC::BYTES, c->stream>>>(
+      c->mapS, P, scalars<T>(c), U, field<T>(c, S_F), field<T>(c, S_ST), field<T>(c, S_UT), field<T>(c, S_XI), zc);
+  prof_close(c, ps_);
+  c->launches++;
 }
 
 template <class T>
@@ -246,13 +271,11 @@ void run_step(cspt_ctx* c) {
   fill_ghosts<T>(c, U, 5, 0);                                                      // O0
   long long n3 = (long long)(L.nx + 6) * (L.ny + 6) * (L.nz + 6);
   long long n2 = (long long)(L.nx + 4) * (L.ny + 4) * (L.nz + 4);
-  long long n1 = (long long)(L.nx + 2) * (L.ny + 2) * (L.nz + 2);
   long long n0 = (long long)L.nx * L.ny * L.nz;
   LAUNCH(c, K_PRIM, k_prim<T>, blocks_for(n3, TPB), TPB, P, U, field<T>(c, S_PR));          // O1
   LAUNCH(c, K_PREDICTOR, k_predictor<T>, blocks_for(n2, TPB), TPB, P, sc, U, field<T>(c, S_PR), field<T>(c, S_F),
-         field<T>(c, S_US), field<T>(c, S_PS));                                    // O3, O4
-  LAUNCH(c, K_CORRECTOR, k_corrector<T>, blocks_for(n1, TPB), TPB, P, sc, U, field<T>(c, S_PR), field<T>(c, S_F),
-         field<T>(c, S_US), field<T>(c, S_PS), field<T>(c, S_UT), field<T>(c, S_XI));   // O5, O6
+         field<T>(c, S_ST));                                                       // O3, O4
+  launch_corrector<T>(c, P, U);                                                    // O5, O6
   LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, sc);
   if (c->legacy_euler)
     LAUNCH(c, K_EULER, k_euler<T>, blocks_for(n0, TPB), TPB, P, sc, U, field<T>(c, S_UT), field<T>(c, S_XI), UN,

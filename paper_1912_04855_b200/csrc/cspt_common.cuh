@@ -51,8 +51,7 @@ enum Slot {
   S_UT = 13,       // U~: mx, my, mz, E  (rho~ = rho^n, G2)      (4)
   S_XI = 17,       // xi^{n+1}                                   (3)
   S_PR = 20,       // primitives of U^n: phi, u, v, w            (4)
-  S_US = 24,       // U*: mx, my, mz, E                          (4)
-  S_PS = 28,       // primitives of U*: phi, u, v, w             (4)
+  S_ST = 24,       // star group: phi*, u*, v*, w*, eta* (3), E* (8)
   S_COUNT = 32
 };
 
@@ -109,8 +108,8 @@ struct cspt_ctx {
   // workspace sub-buffers (byte offsets)
   size_t off_fields, off_inflow, off_scalars;
   long long inflow_plane;  // elements per captured plane
-  // TMA views (x, y, z, field) of the two U buffers and of the (U~, xi) group
-  CUtensorMap mapU[2], mapL;
+  // TMA views (x, y, z, field) of the two U buffers, of the (U~, xi) group and of the star group
+  CUtensorMap mapU[2], mapL, mapS;
   bool have_maps;
   bool legacy_euler;        // debug switch (env CSPT_LEGACY_EULER): first, unfused Euler kernel
   // per-kernel device timing (cspt_profile_*): event pairs recorded around each launch

@@ -74,8 +74,7 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
                const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, T* __restrict__ UN,
                typename Real<T>::bits_t* __restrict__ smax_out, int zchunk) {
   typedef EulerSmem<T, TX, TY> S;
-  extern __shared__ unsigned char smem_raw[];
-  unsigned char* sm = (unsigned char*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+  extern __shared__ __align__(128) unsigned char sm[];
   uint64_t* bar = (uint64_t*)(sm + S::OFF_BAR);
   T* sE = (T*)(sm + S::OFF_E);
   const Layout& L = P.L;

@@ -39,7 +39,7 @@ __global__ void k_prim(Params<T> P, const T* __restrict__ U, T* __restrict__ PR)
 // and Eq. (5), on interior(+)2.
 template <class T>
 __global__ void k_predictor(Params<T> P, const DevScalars<T>* sc, const T* __restrict__ U, const T* __restrict__ PR,
-                            const T* __restrict__ F, T* __restrict__ US, T* __restrict__ PS) {
+                            const T* __restrict__ F, T* __restrict__ ST) {
   const Layout& L = P.L;
   long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   int i, j, k;
@@ -73,72 +73,13 @@ __global__ void k_predictor(Params<T> P, const DevScalars<T>* sc, const T* __res
   T qz = phi_i * sz * P.inv_h + rho * fz;
   T qe = phi_i * se * ((T)0.5 * P.inv_h) + rho * ((ui * fx + vi * fy) + wi * fz);
   T mx = U[c + fs] + dt * qx, my = U[c + 2 * fs] + dt * qy, mz = U[c + 3 * fs] + dt * qz, E = U[c + 4 * fs] + dt * qe;
-  US[c] = mx; US[c + fs] = my; US[c + 2 * fs] = mz; US[c + 3 * fs] = E;
+  // what the corrector needs of (U*, r*): phi*, u*, eta* = xi*/h with xi* = dt/2 (u^n + u*) (Eq. (5),
+  // r^n = centre), and E*; the momentum of U* is rho u* (rho* = rho^n, G2)
   Prim<T> q = prim_fast<T>(rho, mx, my, mz, E, P.gamma, P.rho_vac);
-  PS[c] = q.phi; PS[c + fs] = q.u; PS[c + 2 * fs] = q.v; PS[c + 3 * fs] = q.w;
-}
-
-// -W'(q)/q of the Monaghan cubic spline with smoothing length h (G5).
-template <class T>
-__device__ __forceinline__ T spline_g(T qq) {
-  T t = (T)2 - qq;
-  T g1 = (T)3 - (T)2.25 * qq;
-  T g2 = (T)0.75 * t * t / qq;
-  return qq < (T)1 ? g1 : (qq < (T)2 ? g2 : (T)0);
-}
-
-// O5/O6: HFC{corrector} + SUL{corrector}, Eq. (7) at displaced positions r* and Eq. (6),
-// on interior(+)1.  xi* = dt/2 (u^n + u*) is formed on the fly (Eq. (5), r^n = centre).
-template <class T>
-__global__ void k_corrector(Params<T> P, const DevScalars<T>* sc, const T* __restrict__ U, const T* __restrict__ PR,
-                            const T* __restrict__ F, const T* __restrict__ US, const T* __restrict__ PS,
-                            T* __restrict__ UT, T* __restrict__ XI) {
-  const Layout& L = P.L;
-  long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  int i, j, k;
-  if (!decode_ext(L, 1, m, i, j, k)) return;
-  T dt = load_dt(sc);
-  T hdt = (T)0.5 * dt;
-  long long c = L.idx(i, j, k), fs = L.fstride;
-  T un = PR[c + fs], vn = PR[c + 2 * fs], wn = PR[c + 3 * fs];
-  T ui = PS[c + fs], vi = PS[c + 2 * fs], wi = PS[c + 3 * fs], phi_i = PS[c];
-  T xix = hdt * (un + ui), xiy = hdt * (vn + vi), xiz = hdt * (wn + wi);
-  T sx = 0, sy = 0, sz = 0, se = 0;
-#pragma unroll
-  for (int oz = -1; oz <= 1; ++oz)
-#pragma unroll
-    for (int oy = -1; oy <= 1; ++oy)
-#pragma unroll
-      for (int ox = -1; ox <= 1; ++ox) {
-        if (ox == 0 && oy == 0 && oz == 0) continue;
-        long long cj = c + oz * L.sz() + oy * L.sy() + ox;
-        T uj = PS[cj + fs], vj = PS[cj + 2 * fs], wj = PS[cj + 3 * fs];
-        T dx = -(T)ox * P.h + xix - hdt * (PR[cj + fs] + uj);
-        T dy = -(T)oy * P.h + xiy - hdt * (PR[cj + 2 * fs] + vj);
-        T dz = -(T)oz * P.h + xiz - hdt * (PR[cj + 3 * fs] + wj);
-        T r2 = dx * dx + dy * dy + dz * dz;
-        T qq = sqrt(r2) * P.inv_h;
-        T pw = PS[cj] * spline_g<T>(qq);
-        sx += pw * dx; sy += pw * dy; sz += pw * dz;
-        se += pw * ((ui + uj) * dx + (vi + vj) * dy + (wi + wj) * dz);
-      }
-  T rho = U[c];
-  T fx = F[c], fy = F[c + fs], fz = F[c + 2 * fs];
-  T pn = phi_i * P.wnorm;
-  T qx = pn * sx + rho * fx;
-  T qy = pn * sy + rho * fy;
-  T qz = pn * sz + rho * fz;
-  T qe = (T)0.5 * pn * se + rho * ((ui * fx + vi * fy) + wi * fz);
-  T mx = (T)0.5 * (U[c + fs] + US[c]) + hdt * qx;
-  T my = (T)0.5 * (U[c + 2 * fs] + US[c + fs]) + hdt * qy;
-  T mz = (T)0.5 * (U[c + 3 * fs] + US[c + 2 * fs]) + hdt * qz;
-  T E = (T)0.5 * (U[c + 4 * fs] + US[c + 3 * fs]) + hdt * qe;
-  UT[c] = mx; UT[c + fs] = my; UT[c + 2 * fs] = mz; UT[c + 3 * fs] = E;
-  T ir = rho > P.rho_vac ? (T)1 / rho : (T)0;
-  T qdt = (T)0.25 * dt;
-  XI[c] = (T)0.5 * xix + qdt * (un + mx * ir);
-  XI[c + fs] = (T)0.5 * xiy + qdt * (vn + my * ir);
-  XI[c + 2 * fs] = (T)0.5 * xiz + qdt * (wn + mz * ir);
+  T he = (T)0.5 * dt * P.inv_h;
+  ST[c] = q.phi; ST[c + fs] = q.u; ST[c + 2 * fs] = q.v; ST[c + 3 * fs] = q.w;
+  ST[c + 4 * fs] = he * (ui + q.u); ST[c + 5 * fs] = he * (vi + q.v); ST[c + 6 * fs] = he * (wi + q.w);
+  ST[c + 7 * fs] = E;
 }
 
 template <class T>
