@@ -35,8 +35,7 @@ MIN_WORDS_PER_CELL = 11
 # Algorithmic words per cell of each kernel of the step ("kernels"):
 # the fields a kernel must read once and write once, nothing for stencil re-reads.
 KERNEL_WORDS = {
-    "prim": 5 + 4,                 # U^n -> phi,u,v,w
-    "predictor": 4 + 5 + 3 + 8,    # prim, U^n, f -> star group (phi*, u*, eta*, E*)
+    "predictor": 5 + 3 + 8,        # fused primitives + predictor: U^n, f -> star group (phi*, u*, eta*, E*)
     "corrector": 8 + 5 + 3 + 7,    # star group, U^n, f -> U~, xi
     "euler": 5 + 4 + 3 + 5,        # U^n, U~, xi -> U^{n+1}
     "lagrange": 5 + 3 + 7,         # fused predictor+corrector: U^n, f -> U~, xi

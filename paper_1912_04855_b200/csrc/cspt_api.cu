@@ -70,7 +70,7 @@ constexpr int TPB = 256;
 constexpr int STRIDE_CAP = 148 * 16;   // grid-stride kernels: 16 CTAs of 256 threads per SM
 
 // Event pair around one launch when cspt_profile_enable is on (device time per kernel).
-const char* const kKernelNames[K_COUNT] = {"ghost_fill", "prim", "predictor", "corrector", "euler", "speed_max",
+const char* const kKernelNames[K_COUNT] = {"ghost_fill", "predictor", "corrector", "euler", "speed_max",
                                            "scalar", "io", "force"};
 
 inline int prof_open(cspt_ctx* c, int kid) {
@@ -196,8 +196,6 @@ int compute_dt_t(cspt_ctx* c, double cfl, double* out) {
 }
 
 constexpr int ETX = 32, ETY = 8;     // Euler-stage tile (threads = cells of one plane of the column)
-// corrector tile: CTX x CTY cells per plane, CCY cells (adjacent in y) per thread, CNST ring stages
-constexpr int CTX = 32, CTY = 8, CCY = 2, CNST = 4;
 
 int pick_zchunk(int tiles, int nz) {
   // enough CTAs for ~8 waves of 2 CTAs per SM, but at least 16 planes per CTA (2 extra planes per chunk)
@@ -206,6 +204,40 @@ int pick_zchunk(int tiles, int nz) {
   if (zc < 16) zc = 16;
   if (zc > nz) zc = nz;
   return zc;
+}
+
+// Corrector variants: tile TX x TY cells per plane, CY cells (adjacent in y) per thread, NST ring
+// stages, MINB resident CTAs per SM asked of the compiler.  P == nullptr: set the kernel up (TMA map of
+// the star group, dynamic shared memory); otherwise launch it.
+template <class T, int TX, int TY, int CY, int NST, int MINB>
+bool corr_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
+  typedef CorrSmem<T, TX, TY, CY, NST> SC;
+  const Layout& L = c->L;
+  auto kern = k_corrector_stream<T, TX, TY, CY, NST, MINB>;
+  if (!P) {
+    return make_field_map(&c->mapS, field<T>(c, S_ST), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, SC::NF, SC::BX,
+                          SC::BY, SC::NF) &&
+           cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SC::BYTES) == cudaSuccess;
+  }
+  int gx = (L.nx + 2 + TX - 1) / TX, gy = (L.ny + 2 + TY - 1) / TY;
+  int zc = pick_zchunk(gx * gy, L.nz + 2);
+  dim3 grid(gx, gy, (L.nz + 2 + zc - 1) / zc);
+  int ps_ = prof_open(c, K_CORRECTOR);
+  kern<<<grid, SC::THREADS, SC::BYTES, c->stream>>>(c->mapS, *P, scalars<T>(c), U, field<T>(c, S_F), field<T>(c, S_ST),
+                                                     field<T>(c, S_UT), field<T>(c, S_XI), zc);
+  prof_close(c, ps_);
+  c->launches++;
+  return true;
+}
+
+template <class T>
+bool corr_dispatch(cspt_ctx* c, const Params<T>* P, const T* U) {
+  switch (c->corr_variant) {
+    case 1: return corr_variant<T, 32, 16, 2, 3, 2>(c, P, U);
+    case 2: return corr_variant<T, 32, 8, 1, 4, 2>(c, P, U);
+    case 3: return corr_variant<T, 32, 8, 2, 4, 3>(c, P, U);
+    default: return corr_variant<T, 32, 8, 2, 4, 2>(c, P, U);     // fastest on B200 in both precisions
+  }
 }
 
 template <class T>
@@ -221,29 +253,29 @@ bool make_maps(cspt_ctx* c) {
     ok = cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
          cudaSuccess;
   }
-  typedef CorrSmem<T, CTX, CTY, CCY, CNST> SC;
-  ok = ok && make_field_map(&c->mapS, field<T>(c, S_ST), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, SC::NF, SC::BX,
-                            SC::BY, SC::NF);
-  if (ok) {
-    ok = cudaFuncSetAttribute(k_corrector_stream<T, CTX, CTY, CCY, CNST>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              SC::BYTES) == cudaSuccess;
-  }
+  ok = ok && corr_dispatch<T>(c, nullptr, nullptr);
   return ok;
+}
+
+// primitives + HFC/SUL{predictor} over the extended domain interior(+)2
+constexpr int PTX = 32, PTY = 8;
+template <class T>
+void launch_predictor(cspt_ctx* c, const Params<T>& P, const T* U) {
+  const Layout& L = c->L;
+  int gx = (L.nx + 4 + PTX - 1) / PTX, gy = (L.ny + 4 + PTY - 1) / PTY;
+  int zc = pick_zchunk(gx * gy, L.nz + 4);
+  dim3 grid(gx, gy, (L.nz + 4 + zc - 1) / zc);
+  int ps_ = prof_open(c, K_PREDICTOR);
+  k_predictor_stream<T, PTX, PTY><<<grid, PTX * PTY, 0, c->stream>>>(P, scalars<T>(c), U, field<T>(c, S_F),
+                                                                      field<T>(c, S_ST), zc);
+  prof_close(c, ps_);
+  c->launches++;
 }
 
 // HFC/SUL{corrector} over the extended domain interior(+)1
 template <class T>
 void launch_corrector(cspt_ctx* c, const Params<T>& P, const T* U) {
-  typedef CorrSmem<T, CTX, CTY, CCY, CNST> SC;
-  const Layout& L = c->L;
-  int gx = (L.nx + 2 + CTX - 1) / CTX, gy = (L.ny + 2 + CTY - 1) / CTY;
-  int zc = pick_zchunk(gx * gy, L.nz + 2);
-  dim3 grid(gx, gy, (L.nz + 2 + zc - 1) / zc);
-  int ps_ = prof_open(c, K_CORRECTOR);
-  k_corrector_stream<T, CTX, CTY, CCY, CNST><<<grid, SC::THREADS, SC::BYTES, c->stream>>>(
-      c->mapS, P, scalars<T>(c), U, field<T>(c, S_F), field<T>(c, S_ST), field<T>(c, S_UT), field<T>(c, S_XI), zc);
-  prof_close(c, ps_);
-  c->launches++;
+  corr_dispatch<T>(c, &P, U);
 }
 
 template <class T>
@@ -269,12 +301,8 @@ void run_step(cspt_ctx* c) {
   T* UN = field<T>(c, c->cur ? S_U0 : S_U1);
   DevScalars<T>* sc = scalars<T>(c);
   fill_ghosts<T>(c, U, 5, 0);                                                      // O0
-  long long n3 = (long long)(L.nx + 6) * (L.ny + 6) * (L.nz + 6);
-  long long n2 = (long long)(L.nx + 4) * (L.ny + 4) * (L.nz + 4);
   long long n0 = (long long)L.nx * L.ny * L.nz;
-  LAUNCH(c, K_PRIM, k_prim<T>, blocks_for(n3, TPB), TPB, P, U, field<T>(c, S_PR));          // O1
-  LAUNCH(c, K_PREDICTOR, k_predictor<T>, blocks_for(n2, TPB), TPB, P, sc, U, field<T>(c, S_PR), field<T>(c, S_F),
-         field<T>(c, S_ST));                                                       // O3, O4
+  launch_predictor<T>(c, P, U);                                                    // O1, O3, O4
   launch_corrector<T>(c, P, U);                                                    // O5, O6
   LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, sc);
   if (c->legacy_euler)
@@ -355,6 +383,7 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->stream = (cudaStream_t)cuda_stream;
   carve(c);
   if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
+  c->corr_variant = getenv("CSPT_CORR_VARIANT") ? atoi(getenv("CSPT_CORR_VARIANT")) : 0;   // tuning switch
   c->have_maps = dtype == CSPT_F64 ? make_maps<double>(c) : make_maps<float>(c);
   if (!c->have_maps) { (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }
   c->legacy_euler = getenv("CSPT_LEGACY_EULER") != nullptr;

@@ -50,7 +50,7 @@ enum Slot {
   S_F = 10,        // f = -D[psi]                                (3)
   S_UT = 13,       // U~: mx, my, mz, E  (rho~ = rho^n, G2)      (4)
   S_XI = 17,       // xi^{n+1}                                   (3)
-  S_PR = 20,       // primitives of U^n: phi, u, v, w            (4)
+  S_PR = 20,       // scratch (dense staging of the *_host entry points)  (4)
   S_ST = 24,       // star group: phi*, u*, v*, w*, eta* (3), E* (8)
   S_COUNT = 32
 };
@@ -86,7 +86,7 @@ template <class T> struct DevScalars {
 };
 
 // Kernel ids for cspt_profile_* (names in cspt_api.cu, same order).
-enum KernelId { K_GHOST = 0, K_PRIM, K_PREDICTOR, K_CORRECTOR, K_EULER, K_SPEED_MAX, K_SCALAR, K_IO, K_FORCE, K_COUNT };
+enum KernelId { K_GHOST = 0, K_PREDICTOR, K_CORRECTOR, K_EULER, K_SPEED_MAX, K_SCALAR, K_IO, K_FORCE, K_COUNT };
 
 }  // namespace cspt
 
@@ -111,6 +111,7 @@ struct cspt_ctx {
   // TMA views (x, y, z, field) of the two U buffers, of the (U~, xi) group and of the star group
   CUtensorMap mapU[2], mapL, mapS;
   bool have_maps;
+  int corr_variant;         // tuning switch (env CSPT_CORR_VARIANT): corrector tile variant
   bool legacy_euler;        // debug switch (env CSPT_LEGACY_EULER): first, unfused Euler kernel
   // per-kernel device timing (cspt_profile_*): event pairs recorded around each launch
   bool prof_on;

@@ -33,6 +33,19 @@ template <> struct Fast<double> {
     y = fma(y0, ce, y0);
     t = fma(t0, ce, t0);
   }
+  // 1/x for normal x > 0: MUFU.RCP64H seed + one third-order step, y = y0 (1 + e + e^2), e = 1 - x y0
+  static __device__ __forceinline__ double rcp(double x) {
+    double y0;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
+    double e = fma(-x, y0, 1.0);
+    return fma(y0, fma(e, e, e), y0);
+  }
+  // sqrt(x) for x >= 0; values below 1e-280 (phi < 1e-140) are flushed to 0
+  static __device__ __forceinline__ double sqrt0(double x) {
+    double y, t;
+    rsqrt_sqrt(x, y, t);
+    return x > 1e-280 ? t : 0.0;
+  }
   // comparisons of a positive double with 1 and 4 on the high word (integer pipe)
   static __device__ __forceinline__ bool lt1(double s) { return __double2hiint(s) < 0x3FF00000; }
   static __device__ __forceinline__ bool lt4(double s) { return __double2hiint(s) < 0x40100000; }
@@ -43,6 +56,16 @@ template <> struct Fast<float> {
     asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(s));
     t = s * y;
   }
+  static __device__ __forceinline__ float rcp(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+  }
+  static __device__ __forceinline__ float sqrt0(float x) {
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+  }
   static __device__ __forceinline__ bool lt1(float s) { return s < 1.0f; }
   static __device__ __forceinline__ bool lt4(float s) { return s < 4.0f; }
   static __device__ __forceinline__ float tiny() { return 1e-30f; }
@@ -50,6 +73,159 @@ template <> struct Fast<float> {
 
 // Field order of the star group (slot S_ST): what the predictor hands to the corrector.
 enum StarField { ST_PHI = 0, ST_U, ST_V, ST_W, ST_EX, ST_EY, ST_EZ, ST_E, ST_COUNT };
+
+// ---- O1 + O3 + O4: primitives, HFC{predictor}, SUL{predictor} as one z-streaming kernel -------------
+// Eq. (7) with the particles at the cell centres is the lattice operator
+//   S_c = sum_o a(|o|^2) o_c phi_{i+o},   T = sum_c sum_o a(|o|^2) o_c (phi u_c)_{i+o}
+// (Q_m = -phi_i S / h + rho f,  Q_E = -phi_i (u_i . S + T) / (2h) + rho u_i . f;  G1-G6).
+// One CTA owns a TX x TY column of the extended domain interior(+)2 and streams along z.  Per plane q
+// the threads compute phi, phi u, phi v, phi w of the (TX+2) x (TY+2) cells straight from U^n in
+// global memory into a 2-slot shared-memory buffer; every thread then forms the IN-PLANE parts of the
+// sums of plane q for its column: with the |o_z| = 1 weights they belong to the particles of planes
+// q-1 and q+1 (sign of the z terms flipped), with the o_z = 0 weights to plane q.  The running sums
+// of the two particles in flight live in registers; particle q-1 is finished (Eq. (5)) when plane q
+// has been added.  Output: the star group the corrector reads (phi*, u*, eta*, E*).
+template <class T>
+__device__ __forceinline__ Prim<T> prim_quick(T rho, T mx, T my, T mz, T E, T gamma, T rho_vac) {
+  typedef Fast<T> FT;
+  Prim<T> q;
+  q.ok = rho > rho_vac;
+  T ir = q.ok ? FT::rcp(rho) : (T)0;
+  q.u = mx * ir; q.v = my * ir; q.w = mz * ir;
+  T ke2 = (mx * q.u + my * q.v) + mz * q.w;
+  T pp = (gamma - (T)1) * (E - (T)0.5 * ke2);
+  q.p = q.ok ? (pp > (T)0 ? pp : (T)0) : (T)0;
+  q.phi = FT::sqrt0((T)2 * q.p);
+  return q;
+}
+
+template <class T, int TX, int TY>
+struct PredSmem {
+  static constexpr int BX = TX + 2, BY = TY + 2;
+  static constexpr int NHALO = BX * BY - TX * TY;
+  static constexpr int PLANE = 4 * BY * BX;              // phi, phi u, phi v, phi w
+  static_assert(NHALO <= TX * TY, "one halo cell per thread at most");
+};
+
+template <class T, int TX, int TY>
+__global__ void __launch_bounds__(TX* TY)
+k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, const T* __restrict__ F,
+                   T* __restrict__ ST, int zchunk) {
+  typedef PredSmem<T, TX, TY> S;
+  __shared__ T sbuf[2][S::PLANE];
+  const Layout& L = P.L;
+  const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
+  const int i0 = -2 + (int)blockIdx.x * TX, j0 = -2 + (int)blockIdx.y * TY;
+  const int z0 = -2 + (int)blockIdx.z * zchunk, z1 = min(L.nz + 2, z0 + zchunk);   // particle planes [z0, z1)
+  const long long fs = L.fstride;
+  // own cell: its primitives are needed up to ghost layer 3 (neighbour of the last particle), the
+  // particle itself exists up to layer 2; beyond that the index is clamped and the result unused
+  const int i = min(i0 + tx, L.nx + 2), j = min(j0 + ty, L.ny + 2);
+  const bool valid = (i0 + tx) <= L.nx + 1 && (j0 + ty) <= L.ny + 1;
+  // halo cell of this thread (tile coordinates -1..TX, -1..TY)
+  const bool has_halo = tid < S::NHALO;
+  int hx, hy;
+  if (tid < S::BX) { hx = tid - 1; hy = -1; }
+  else if (tid < 2 * S::BX) { hx = tid - S::BX - 1; hy = TY; }
+  else { int t = tid - 2 * S::BX; hx = (t & 1) ? TX : -1; hy = t >> 1; }
+  const int hi = min(i0 + hx, L.nx + 2), hj = min(j0 + hy, L.ny + 2);
+  const long long c_own = L.idx(i, j, 0), c_halo = L.idx(hi, hj, 0), sz = L.sz();
+
+  const T dt = load_dt(sc);
+  const T he = (T)0.5 * dt * P.inv_h;
+  const T a1 = P.a1, a2 = P.a2, a3 = P.a3;
+
+  auto put = [&](T* sb, int ly, int lx, const Prim<T>& q) {
+    int o = (ly + 1) * S::BX + (lx + 1);
+    sb[o] = q.phi; sb[S::BY * S::BX + o] = q.phi * q.u; sb[2 * S::BY * S::BX + o] = q.phi * q.v;
+    sb[3 * S::BY * S::BX + o] = q.phi * q.w;
+  };
+
+  T Uo[5], Uh[5];                 // plane q: own and halo cell, loaded one iteration ahead
+  {
+    const long long co = c_own + (long long)(z0 - 1) * sz, ch = c_halo + (long long)(z0 - 1) * sz;
+#pragma unroll
+    for (int f = 0; f < 5; ++f) { Uo[f] = __ldg(U + co + f * fs); Uh[f] = has_halo ? __ldg(U + ch + f * fs) : (T)0; }
+  }
+  T Uc[5] = {0, 0, 0, 0, 0};      // particle q-1: U^n and primitives
+  Prim<T> pc; pc.u = pc.v = pc.w = pc.p = pc.phi = (T)0; pc.ok = false;
+  T acc0[4] = {0, 0, 0, 0}, acc1[4] = {0, 0, 0, 0};
+
+  for (int q = z0 - 1; q <= z1; ++q) {
+    T* sb = sbuf[(q - (z0 - 1)) & 1];
+    // O1 for plane q
+    Prim<T> po = prim_quick<T>(Uo[0], Uo[1], Uo[2], Uo[3], Uo[4], P.gamma, P.rho_vac);
+    put(sb, ty, tx, po);
+    if (has_halo) {
+      Prim<T> ph = prim_quick<T>(Uh[0], Uh[1], Uh[2], Uh[3], Uh[4], P.gamma, P.rho_vac);
+      put(sb, hy, hx, ph);
+    }
+    T Un[5];
+#pragma unroll
+    for (int f = 0; f < 5; ++f) Un[f] = Uo[f];
+    // request plane q+1 and the force of particle q-1
+    T fq[3] = {0, 0, 0};
+    if (q < z1) {
+      const long long co = c_own + (long long)(q + 1) * sz, ch = c_halo + (long long)(q + 1) * sz;
+#pragma unroll
+      for (int f = 0; f < 5; ++f) { Uo[f] = __ldg(U + co + f * fs); if (has_halo) Uh[f] = __ldg(U + ch + f * fs); }
+    }
+    const long long cs = c_own + (long long)(q - 1) * sz;       // particle q-1
+    if (q - 1 >= z0) {
+#pragma unroll
+      for (int f = 0; f < 3; ++f) fq[f] = __ldg(F + cs + f * fs);
+    }
+    __syncthreads();
+
+    // in-plane parts of the lattice sums of plane q (tile coordinates of the own column: tx, ty)
+    auto at = [&](int f, int oy, int ox) { return sb[(f * S::BY + (ty + 1 + oy)) * S::BX + (tx + 1 + ox)]; };
+    T A0x, A0y, T0, A1x, A1y, A1z, T1xy, T1z;
+    {
+      // phi: x and y differences, and the plain 3x3 sum
+      T pmm = at(0, -1, -1), pm0 = at(0, -1, 0), pmp = at(0, -1, 1);
+      T p0m = at(0, 0, -1), p00 = at(0, 0, 0), p0p = at(0, 0, 1);
+      T ppm = at(0, 1, -1), pp0 = at(0, 1, 0), ppp = at(0, 1, 1);
+      T dx0 = p0p - p0m, dxs = (pmp - pmm) + (ppp - ppm);        // o_y = 0; o_y = +-1
+      T dy0 = pp0 - pm0, dys = (ppm - pmm) + (ppp - pmp);        // o_x = 0; o_x = +-1
+      A0x = a1 * dx0 + a2 * dxs;  A1x = a2 * dx0 + a3 * dxs;
+      A0y = a1 * dy0 + a2 * dys;  A1y = a2 * dy0 + a3 * dys;
+      A1z = a1 * p00 + a2 * ((p0m + p0p) + (pm0 + pp0)) + a3 * ((pmm + pmp) + (ppm + ppp));
+      // phi u: x differences;  phi v: y differences
+      T ux0 = at(1, 0, 1) - at(1, 0, -1), uxs = (at(1, -1, 1) - at(1, -1, -1)) + (at(1, 1, 1) - at(1, 1, -1));
+      T vy0 = at(2, 1, 0) - at(2, -1, 0), vys = (at(2, 1, -1) - at(2, -1, -1)) + (at(2, 1, 1) - at(2, -1, 1));
+      T0 = a1 * (ux0 + vy0) + a2 * (uxs + vys);
+      T1xy = a2 * (ux0 + vy0) + a3 * (uxs + vys);
+      // phi w: plain 3x3 sum
+      T1z = a1 * at(3, 0, 0) + a2 * ((at(3, 0, -1) + at(3, 0, 1)) + (at(3, -1, 0) + at(3, 1, 0))) +
+            a3 * ((at(3, -1, -1) + at(3, -1, 1)) + (at(3, 1, -1) + at(3, 1, 1)));
+    }
+
+    // particle q-1: plane q is its o_z = +1 layer; Eq. (7) and Eq. (5)
+    if (q - 1 >= z0 && valid) {
+      const T Sx = acc0[0] + A1x, Sy = acc0[1] + A1y, Sz = acc0[2] + A1z, Tt = acc0[3] + (T1xy + T1z);
+      const T rho = Uc[0];
+      const T ui = pc.u, vi = pc.v, wi = pc.w;
+      const T pn = pc.phi * P.inv_h;
+      const T qx = rho * fq[0] - pn * Sx;
+      const T qy = rho * fq[1] - pn * Sy;
+      const T qz = rho * fq[2] - pn * Sz;
+      const T qe = rho * ((ui * fq[0] + vi * fq[1]) + wi * fq[2]) - (T)0.5 * pn * (((ui * Sx + vi * Sy) + wi * Sz) + Tt);
+      const T mx = Uc[1] + dt * qx, my = Uc[2] + dt * qy, mz = Uc[3] + dt * qz, E = Uc[4] + dt * qe;
+      Prim<T> ps = prim_quick<T>(rho, mx, my, mz, E, P.gamma, P.rho_vac);
+      ST[cs] = ps.phi; ST[cs + fs] = ps.u; ST[cs + 2 * fs] = ps.v; ST[cs + 3 * fs] = ps.w;
+      ST[cs + 4 * fs] = he * (ui + ps.u); ST[cs + 5 * fs] = he * (vi + ps.v); ST[cs + 6 * fs] = he * (wi + ps.w);
+      ST[cs + 7 * fs] = E;
+    }
+    // particle q: had plane q-1 as its o_z = -1 layer, plane q is its own layer
+    acc0[0] = acc1[0] + A0x; acc0[1] = acc1[1] + A0y; acc0[2] = acc1[2]; acc0[3] = acc1[3] + T0;
+    // particle q+1: plane q is its o_z = -1 layer
+    acc1[0] = A1x; acc1[1] = A1y; acc1[2] = -A1z; acc1[3] = T1xy - T1z;
+#pragma unroll
+    for (int f = 0; f < 5; ++f) Uc[f] = Un[f];
+    pc = po;
+  }
+}
+
 
 template <class T, int TX, int TY, int CY, int NST>
 struct CorrSmem {
@@ -68,8 +244,8 @@ struct CorrSmem {
   static_assert((BX * sizeof(T)) % 16 == 0, "box rows must be multiples of 16 bytes");
 };
 
-template <class T, int TX, int TY, int CY, int NST>
-__global__ void __launch_bounds__(TX*(TY / CY))
+template <class T, int TX, int TY, int CY, int NST, int MINB>
+__global__ void __launch_bounds__(TX*(TY / CY), MINB)
 k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const DevScalars<T>* __restrict__ sc,
                    const T* __restrict__ U, const T* __restrict__ F, const T* __restrict__ ST, T* __restrict__ UT,
                    T* __restrict__ XI, int zchunk) {
@@ -142,6 +318,18 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
     bool any = false;
 #pragma unroll
     for (int c = 0; c < CY; ++c) any = any || valid[c];
+    // own-cell operands of Eq. (6) straight from global memory, requested before the neighbour loop
+    // so that their latency is hidden behind it
+    T own[CY][9];
+#pragma unroll
+    for (int c = 0; c < CY; ++c) {
+      const long long cc = L.idx(valid[c] ? i : 0, valid[c] ? j0 + ly0 + c : 0, p);
+#pragma unroll
+      for (int f = 0; f < 5; ++f) own[c][f] = __ldg(U + cc + f * fs);
+#pragma unroll
+      for (int f = 0; f < 3; ++f) own[c][5 + f] = __ldg(F + cc + f * fs);
+      own[c][8] = __ldg(ST + cc + (long long)ST_E * fs);
+    }
 
     if (any) {
 #pragma unroll
@@ -189,9 +377,9 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
       if (!valid[c]) continue;
       const int j = j0 + ly0 + c;
       const long long cc = L.idx(i, j, p);
-      const T rho = U[cc], mxn = U[cc + fs], myn = U[cc + 2 * fs], mzn = U[cc + 3 * fs], En = U[cc + 4 * fs];
-      const T fx = F[cc], fy = F[cc + fs], fz = F[cc + 2 * fs];
-      const T Es = ST[cc + (long long)ST_E * fs];
+      const T rho = own[c][0], mxn = own[c][1], myn = own[c][2], mzn = own[c][3], En = own[c][4];
+      const T fx = own[c][5], fy = own[c][6], fz = own[c][7];
+      const T Es = own[c][8];
       const bool ok = rho > P.rho_vac;
       const T ir = ok ? (T)1 / rho : (T)0;
       const T un = mxn * ir, vn = myn * ir, wn = mzn * ir;

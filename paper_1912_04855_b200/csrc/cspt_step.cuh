@@ -1,6 +1,6 @@
-// cspt_step.cuh -- the step kernels: HFC/SUL predictor, HFC/SUL corrector, FGC+SUE.
-// (Eq. (4)-(8)).  First, straightforward version: one thread per
-// cell, stencil operands read through L1/L2.
+// cspt_step.cuh -- helpers shared by the step kernels, and the straightforward (one thread per
+// cell, operands through L1/L2) FGC+SUE kernel kept as a debugging cross-check (env CSPT_LEGACY_EULER).
+// (Eq. (4)-(8)).
 #pragma once
 #include "cspt_kernels.cuh"
 
@@ -21,65 +21,6 @@ template <class T>
 __device__ __forceinline__ T load_dt(const DevScalars<T>* sc) {
   T dt = sc->dt;
   return dt < Real<T>::inf() ? dt : (T)0;       // all-vacuum grid: dt = +inf -> identity step
-}
-
-// O1 on the whole padded array: phi, u, v, w of U^n.
-template <class T>
-__global__ void k_prim(Params<T> P, const T* __restrict__ U, T* __restrict__ PR) {
-  const Layout& L = P.L;
-  long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  int i, j, k;
-  if (!decode_ext(L, NG, m, i, j, k)) return;
-  long long c = L.idx(i, j, k), fs = L.fstride;
-  Prim<T> q = prim_fast<T>(U[c], U[c + fs], U[c + 2 * fs], U[c + 3 * fs], U[c + 4 * fs], P.gamma, P.rho_vac);
-  PR[c] = q.phi; PR[c + fs] = q.u; PR[c + 2 * fs] = q.v; PR[c + 3 * fs] = q.w;
-}
-
-// O3+O4: HFC{predictor} + SUL{predictor}, Eq. (7) with particles at the cell centres
-// and Eq. (5), on interior(+)2.
-template <class T>
-__global__ void k_predictor(Params<T> P, const DevScalars<T>* sc, const T* __restrict__ U, const T* __restrict__ PR,
-                            const T* __restrict__ F, T* __restrict__ ST) {
-  const Layout& L = P.L;
-  long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  int i, j, k;
-  if (!decode_ext(L, 2, m, i, j, k)) return;
-  T dt = load_dt(sc);
-  long long c = L.idx(i, j, k), fs = L.fstride;
-  T ui = PR[c + fs], vi = PR[c + 2 * fs], wi = PR[c + 3 * fs], phi_i = PR[c];
-  T sx = 0, sy = 0, sz = 0, se = 0;
-#pragma unroll
-  for (int oz = -1; oz <= 1; ++oz)
-#pragma unroll
-    for (int oy = -1; oy <= 1; ++oy)
-#pragma unroll
-      for (int ox = -1; ox <= 1; ++ox) {
-        int o2 = ox * ox + oy * oy + oz * oz;
-        if (o2 == 0) continue;
-        T a = o2 == 1 ? P.a1 : (o2 == 2 ? P.a2 : P.a3);
-        long long cj = c + oz * L.sz() + oy * L.sy() + ox;
-        T pw = PR[cj] * a;                      // phi_j * a(|o|^2); d = -o h
-        T ud = (T)0;
-        if (ox) { sx -= (T)ox * pw; ud -= (T)ox * (ui + PR[cj + fs]); }
-        if (oy) { sy -= (T)oy * pw; ud -= (T)oy * (vi + PR[cj + 2 * fs]); }
-        if (oz) { sz -= (T)oz * pw; ud -= (T)oz * (wi + PR[cj + 3 * fs]); }
-        se += pw * ud;
-      }
-  T rho = U[c];
-  T fx = F[c], fy = F[c + fs], fz = F[c + 2 * fs];
-  // S = (1/h) * sum a o phi_j  (sign folded above); Q per G1
-  T qx = phi_i * sx * P.inv_h + rho * fx;
-  T qy = phi_i * sy * P.inv_h + rho * fy;
-  T qz = phi_i * sz * P.inv_h + rho * fz;
-  T qe = phi_i * se * ((T)0.5 * P.inv_h) + rho * ((ui * fx + vi * fy) + wi * fz);
-  T mx = U[c + fs] + dt * qx, my = U[c + 2 * fs] + dt * qy, mz = U[c + 3 * fs] + dt * qz, E = U[c + 4 * fs] + dt * qe;
-  // what the corrector needs of (U*, r*): phi*, u*, eta* = xi*/h with xi* = dt/2 (u^n + u*) (Eq. (5),
-  // r^n = centre), and E*; the momentum of U* is rho u* (rho* = rho^n, G2)
-  Prim<T> q = prim_fast<T>(rho, mx, my, mz, E, P.gamma, P.rho_vac);
-  T he = (T)0.5 * dt * P.inv_h;
-  ST[c] = q.phi; ST[c + fs] = q.u; ST[c + 2 * fs] = q.v; ST[c + 3 * fs] = q.w;
-  ST[c + 4 * fs] = he * (ui + q.u); ST[c + 5 * fs] = he * (vi + q.v); ST[c + 6 * fs] = he * (wi + q.w);
-  ST[c + 7 * fs] = E;
 }
 
 template <class T>
