@@ -115,15 +115,21 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
     for (int q = 0; q < 5; ++q) { Um[q] = inside ? U[c + q * fs] : (T)0; FPzp[q] = 0; acc[q] = 0; Utp[q] = 0; }
   }
 
+  // own column of plane p+1 comes straight from global memory (it becomes a TMA box one iteration
+  // later); it is requested a full iteration ahead so that its latency is hidden
+  const long long c_col = L.idx(inside ? i : 0, inside ? j : 0, 0), szp = L.sz();
+  T Unext[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) Unext[q] = __ldg(U + c_col + (long long)z0 * szp + q * fs);
   uint32_t phase = 0;        // bit s: parity to wait for on stage s
   for (int p = z0 - 1; p <= z1; ++p) {
     const int s = (p - (z0 - 1)) & 1;
-    // own column of plane p+1 straight from global (it becomes a TMA box one iteration later)
     T Up[5];
-    {
-      long long c = L.idx(inside ? i : 0, inside ? j : 0, p + 1);
 #pragma unroll
-      for (int q = 0; q < 5; ++q) Up[q] = inside ? __ldg(U + c + q * fs) : (T)0;
+    for (int q = 0; q < 5; ++q) Up[q] = Unext[q];
+    if (p < z1) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) Unext[q] = __ldg(U + c_col + (long long)(p + 2) * szp + q * fs);
     }
     mbar_wait(&bar[s], (phase >> s) & 1u);
     phase ^= 1u << s;

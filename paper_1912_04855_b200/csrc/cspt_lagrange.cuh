@@ -147,6 +147,7 @@ k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* _
 #pragma unroll
     for (int f = 0; f < 5; ++f) { Uo[f] = __ldg(U + co + f * fs); Uh[f] = has_halo ? __ldg(U + ch + f * fs) : (T)0; }
   }
+  T fn[3] = {0, 0, 0};            // force of particle q, requested one iteration before it is needed
   T Uc[5] = {0, 0, 0, 0, 0};      // particle q-1: U^n and primitives
   Prim<T> pc; pc.u = pc.v = pc.w = pc.p = pc.phi = (T)0; pc.ok = false;
   T acc0[4] = {0, 0, 0, 0}, acc1[4] = {0, 0, 0, 0};
@@ -163,18 +164,21 @@ k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* _
     T Un[5];
 #pragma unroll
     for (int f = 0; f < 5; ++f) Un[f] = Uo[f];
-    // request plane q+1 and the force of particle q-1
-    T fq[3] = {0, 0, 0};
+    // request plane q+1 and the force of particle q (used in the next iteration)
+    T fq[3];
+#pragma unroll
+    for (int f = 0; f < 3; ++f) fq[f] = fn[f];
     if (q < z1) {
       const long long co = c_own + (long long)(q + 1) * sz, ch = c_halo + (long long)(q + 1) * sz;
 #pragma unroll
       for (int f = 0; f < 5; ++f) { Uo[f] = __ldg(U + co + f * fs); if (has_halo) Uh[f] = __ldg(U + ch + f * fs); }
+      if (q >= z0) {
+        const long long cf = c_own + (long long)q * sz;
+#pragma unroll
+        for (int f = 0; f < 3; ++f) fn[f] = __ldg(F + cf + f * fs);
+      }
     }
     const long long cs = c_own + (long long)(q - 1) * sz;       // particle q-1
-    if (q - 1 >= z0) {
-#pragma unroll
-      for (int f = 0; f < 3; ++f) fq[f] = __ldg(F + cs + f * fs);
-    }
     __syncthreads();
 
     // in-plane parts of the lattice sums of plane q (tile coordinates of the own column: tx, ty)
