@@ -6,6 +6,7 @@
 
 #include "cspt_step.cuh"
 #include "cspt_euler.cuh"
+#include "cspt_euler_block.cuh"
 #include "cspt_lagrange.cuh"
 
 using namespace cspt;
@@ -195,7 +196,10 @@ int compute_dt_t(cspt_ctx* c, double cfl, double* out) {
   return CSPT_OK;
 }
 
-constexpr int ETX = 32, ETY = 8;     // Euler-stage tile (threads = cells of one plane of the column)
+// Euler-stage tile: one warp per row plus two halo-row warps; 6 rows in fp64 (8 warps, 128 registers
+// per thread at 2 CTAs per SM), 8 rows in fp32
+constexpr int ETX = 32;
+template <class T> struct EulerTile { static constexpr int TY = 8; };
 
 int pick_zchunk(int tiles, int nz) {
   // enough CTAs for ~8 waves of 2 CTAs per SM, but at least 16 planes per CTA (2 extra planes per chunk)
@@ -243,15 +247,20 @@ bool corr_dispatch(cspt_ctx* c, const Params<T>* P, const T* U) {
 template <class T>
 bool make_maps(cspt_ctx* c) {
   const Layout& L = c->L;
-  typedef EulerSmem<T, ETX, ETY> S;
+  typedef EulerSmem<T, ETX, EulerTile<T>::TY> S;
+  constexpr int ETY = EulerTile<T>::TY;
   bool ok = true;
   for (int b = 0; b < 2; ++b)
     ok = ok && make_field_map(&c->mapU[b], field<T>(c, b ? S_U1 : S_U0), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 5,
                               S::BX, S::UY, 5);
   ok = ok && make_field_map(&c->mapL, field<T>(c, S_UT), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 7, S::BX, S::LY, 7);
   if (ok) {
+    // both layouts of the stage read the same boxes (TX x TY tile, halo 2 / 1)
+    static_assert(EulerSmemB<T, ETX, ETY>::BX == S::BX && EulerSmemB<T, ETX, ETY>::UY == S::UY, "same TMA boxes");
     ok = cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
-         cudaSuccess;
+             cudaSuccess &&
+         cudaFuncSetAttribute(k_euler_block<T, ETX, ETY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              EulerSmemB<T, ETX, ETY>::BYTES) == cudaSuccess;
   }
   ok = ok && corr_dispatch<T>(c, nullptr, nullptr);
   return ok;
@@ -280,15 +289,22 @@ void launch_corrector(cspt_ctx* c, const Params<T>& P, const T* U) {
 
 template <class T>
 void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
-  typedef EulerSmem<T, ETX, ETY> S;
+  typedef EulerSmem<T, ETX, EulerTile<T>::TY> S;
+  constexpr int ETY = EulerTile<T>::TY;
   const Layout& L = c->L;
   int gx = (L.nx + ETX - 1) / ETX, gy = (L.ny + ETY - 1) / ETY;
   int zc = pick_zchunk(gx * gy, L.nz);
   dim3 grid(gx, gy, (L.nz + zc - 1) / zc);
   DevScalars<T>* sc = scalars<T>(c);
   int ps_ = prof_open(c, K_EULER);
-  k_euler_stream<T, ETX, ETY><<<grid, ETX * ETY, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN,
-                                                                         &sc->smax_bits, zc);
+  if (c->euler_variant == 1) {
+    typedef EulerSmemB<T, ETX, ETY> SB;
+    k_euler_block<T, ETX, ETY><<<grid, ETX * ETY, SB::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN,
+                                                                          &sc->smax_bits, zc);
+  } else {
+    k_euler_stream<T, ETX, ETY><<<grid, S::THREADS, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN,
+                                                                           &sc->smax_bits, zc);
+  }
   prof_close(c, ps_);
   c->launches++;
 }
@@ -387,6 +403,8 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->have_maps = dtype == CSPT_F64 ? make_maps<double>(c) : make_maps<float>(c);
   if (!c->have_maps) { (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }
   c->legacy_euler = getenv("CSPT_LEGACY_EULER") != nullptr;
+  // layout of the Euler stage: block layout in fp64, halo-warp layout in fp32 (measured on B200); tuning switch
+  c->euler_variant = getenv("CSPT_EULER_VARIANT") ? atoi(getenv("CSPT_EULER_VARIANT")) : (dtype == CSPT_F64 ? 1 : 0);
   *out = c;
   return CSPT_OK;
 }

@@ -1,0 +1,218 @@
+// cspt_euler_block.cuh -- FGC + SUE, second layout of the same stage (see cspt_euler.cuh for the
+// method): TX x TY threads = cells of one plane of the column, no halo warps; the one-sided flux parts
+// go to the x and to the y neighbours through shared memory (the halo columns / rows are computed by
+// the first and the last warps), four barriers per plane.  Faster than the halo-warp layout in fp64
+// (128 registers per thread at 2 CTAs per SM), slower in fp32.
+#pragma once
+#include "cspt_euler.cuh"
+
+namespace cspt {
+
+template <class T, int TX, int TY>
+struct EulerSmemB {
+  // x halo of the boxes: 2 cells are needed; 16 bytes' worth are loaded so that every box row starts
+  // on a 16-byte boundary in global memory (an 8-byte-aligned fp32 start raised "illegal instruction")
+  static constexpr int HX = 16 / (int)sizeof(T) < 2 ? 2 : 16 / (int)sizeof(T);
+  static constexpr int BX = TX + 2 * HX;
+  static constexpr int UY = TY + 4, LY = TY + 2;
+  static constexpr int U_ELEMS = 5 * UY * BX;
+  static constexpr int L_ELEMS = 7 * LY * BX;
+  static constexpr int U_STAGE = (U_ELEMS * (int)sizeof(T) + 127) / 128 * 128;    // bytes
+  static constexpr int L_STAGE = (L_ELEMS * (int)sizeof(T) + 127) / 128 * 128;
+  static constexpr int EX_ELEMS = 10 * (TX + 2) * (TY + 2);                       // exchange buffer (x, then y)
+  static constexpr int OFF_U = 0;
+  static constexpr int OFF_L = OFF_U + 2 * U_STAGE;
+  static constexpr int OFF_E = OFF_L + 2 * L_STAGE;
+  static constexpr int OFF_BAR = OFF_E + (EX_ELEMS * (int)sizeof(T) + 127) / 128 * 128;
+  static constexpr int BYTES = OFF_BAR + 64 + 128;  // + slack for the 128-byte alignment of the base
+};
+
+template <class T, int TX, int TY>
+__global__ void __launch_bounds__(TX* TY, 2)
+k_euler_block(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL, Params<T> P,
+               const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, T* __restrict__ UN,
+               typename Real<T>::bits_t* __restrict__ smax_out, int zchunk) {
+  typedef EulerSmemB<T, TX, TY> S;
+  extern __shared__ __align__(128) unsigned char sm[];
+  uint64_t* bar = (uint64_t*)(sm + S::OFF_BAR);
+  T* sE = (T*)(sm + S::OFF_E);
+  const Layout& L = P.L;
+  const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
+  const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
+  const int z0 = blockIdx.z * zchunk, z1 = min(L.nz, z0 + zchunk);
+  const int i = i0 + tx, j = j0 + ty;
+  const bool inside = i < L.nx && j < L.ny;
+  const long long fs = L.fstride;
+  constexpr uint32_t TX_BYTES = (uint32_t)((S::U_ELEMS + S::L_ELEMS) * sizeof(T));
+
+  if (tid == 0) {
+    mbar_init(&bar[0], 1);
+    mbar_init(&bar[1], 1);
+    mbar_fence_init();
+    prefetch_tmap(&mapU);
+    prefetch_tmap(&mapL);
+  }
+  __syncthreads();
+  auto issue = [&](int p, int s) {      // plane p -> stage s
+    mbar_expect_tx(&bar[s], TX_BYTES);
+    tma_load_4d(sm + S::OFF_U + s * S::U_STAGE, &mapU, &bar[s], i0 + GX - S::HX, j0 + NG - 2, p + NG, 0);
+    tma_load_4d(sm + S::OFF_L + s * S::L_STAGE, &mapL, &bar[s], i0 + GX - S::HX, j0 + NG - 1, p + NG, 0);
+  };
+  if (tid == 0) {
+    issue(z0 - 1, 0);
+    issue(z0, 1);
+  }
+
+  const T dt = load_dt(sc);
+  const T lam = dt * P.inv_h;
+  T Um[5], FPzp[5], acc[5], Utp[5];
+  T smax = 0;
+  // U^n of plane z0-2 (own column) for the z slope of plane z0-1
+  {
+    long long c = L.idx(inside ? i : 0, inside ? j : 0, z0 - 2);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { Um[q] = inside ? U[c + q * fs] : (T)0; FPzp[q] = 0; acc[q] = 0; Utp[q] = 0; }
+  }
+
+  // own column of plane p+1 comes straight from global memory (it becomes a TMA box one iteration
+  // later); it is requested a full iteration ahead so that its latency is hidden
+  const long long c_col = L.idx(inside ? i : 0, inside ? j : 0, 0), szp = L.sz();
+  T Unext[5];
+#pragma unroll
+  for (int q = 0; q < 5; ++q) Unext[q] = __ldg(U + c_col + (long long)z0 * szp + q * fs);
+  uint32_t phase = 0;        // bit s: parity to wait for on stage s
+  for (int p = z0 - 1; p <= z1; ++p) {
+    const int s = (p - (z0 - 1)) & 1;
+    T Up[5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) Up[q] = Unext[q];
+    if (p < z1) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) Unext[q] = __ldg(U + c_col + (long long)(p + 2) * szp + q * fs);
+    }
+    mbar_wait(&bar[s], (phase >> s) & 1u);
+    phase ^= 1u << s;
+    const T* sU = (const T*)(sm + S::OFF_U + s * S::U_STAGE);
+    const T* sL = (const T*)(sm + S::OFF_L + s * S::L_STAGE);
+    auto u_at = [&](int q, int y, int x) { return sU[(q * S::UY + (y + 2)) * S::BX + (x + S::HX)]; };   // tile coords
+    auto l_at = [&](int q, int y, int x) { return sL[(q * S::LY + (y + 1)) * S::BX + (x + S::HX)]; };
+
+    T U0[5], hf[5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) U0[q] = u_at(q, ty, tx);
+    hf[0] = U0[0];                                              // rho~ = rho^n (G2)
+#pragma unroll
+    for (int q = 1; q < 5; ++q) hf[q] = (T)0.5 * (U0[q] + l_at(q - 1, ty, tx));
+
+    // z axis: both parts of plane p
+    T FPz[5], FMz[5];
+    flux_parts<T, 3>(P, 2, U0, Um, Up, hf, l_at(6, ty, tx), FPz, FMz);
+
+    // finish cell p-1 (SUE, Eq. (4))
+    if (p - 1 >= z0) {
+      T un[5];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) un[q] = Utp[q] - lam * (acc[q] + FMz[q]);
+      if (inside) {
+        long long c = L.idx(i, j, p - 1);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) UN[c + q * fs] = un[q];
+        T sp = cell_speed_exact<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
+        smax = sp > smax ? sp : smax;
+      }
+    }
+
+    if (p >= z0 && p < z1) {
+      T a[5];
+      // ---- x axis -------------------------------------------------------------
+      {
+        T Ux0[5], Ux1[5], FP[5], FM[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { Ux0[q] = u_at(q, ty, tx - 1); Ux1[q] = u_at(q, ty, tx + 1); }
+        flux_parts<T, 3>(P, 0, U0, Ux0, Ux1, hf, l_at(4, ty, tx), FP, FM);
+        // exchange layout: [q][ty][tx+1], FP in 0..4, FM in 5..9, row pitch TX+2
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          sE[(q * TY + ty) * (TX + 2) + tx + 1] = FP[q];
+          sE[((q + 5) * TY + ty) * (TX + 2) + tx + 1] = FM[q];
+          a[q] = FP[q] - FM[q];
+        }
+        if (tid < 2 * TY) {                         // halo columns x = -1 (FP only) and x = TX (FM only)
+          int hy = tid >> 1, side = tid & 1, hx = side ? TX : -1;
+          T Hc[5], Hm[5], Hp[5], hh[5], HF[5];
+#pragma unroll
+          for (int q = 0; q < 5; ++q) { Hc[q] = u_at(q, hy, hx); Hm[q] = u_at(q, hy, hx - 1); Hp[q] = u_at(q, hy, hx + 1); }
+          hh[0] = Hc[0];
+#pragma unroll
+          for (int q = 1; q < 5; ++q) hh[q] = (T)0.5 * (Hc[q] + l_at(q - 1, hy, hx));
+          T hxi = l_at(4, hy, hx);
+          if (side) {
+            flux_parts<T, 2>(P, 0, Hc, Hm, Hp, hh, hxi, HF, HF);
+#pragma unroll
+            for (int q = 0; q < 5; ++q) sE[((q + 5) * TY + hy) * (TX + 2) + TX + 1] = HF[q];
+          } else {
+            flux_parts<T, 1>(P, 0, Hc, Hm, Hp, hh, hxi, HF, HF);
+#pragma unroll
+            for (int q = 0; q < 5; ++q) sE[(q * TY + hy) * (TX + 2) + 0] = HF[q];
+          }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 5; ++q)
+          a[q] += sE[((q + 5) * TY + ty) * (TX + 2) + tx + 2] - sE[(q * TY + ty) * (TX + 2) + tx];
+        __syncthreads();
+      }
+      // ---- y axis -------------------------------------------------------------
+      {
+        T Uy0[5], Uy1[5], FP[5], FM[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { Uy0[q] = u_at(q, ty - 1, tx); Uy1[q] = u_at(q, ty + 1, tx); }
+        flux_parts<T, 3>(P, 1, U0, Uy0, Uy1, hf, l_at(5, ty, tx), FP, FM);
+        // exchange layout: [q][ty+1][tx], rows -1..TY, row pitch TX
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          sE[(q * (TY + 2) + ty + 1) * TX + tx] = FP[q];
+          sE[((q + 5) * (TY + 2) + ty + 1) * TX + tx] = FM[q];
+          a[q] += FP[q] - FM[q];
+        }
+        if (tid >= TX * TY - 2 * TX) {               // halo rows y = -1 (FP only) and y = TY (FM only): last two warps
+          int t = tid - (TX * TY - 2 * TX);
+          int hx = t % TX, side = t / TX, hy = side ? TY : -1;
+          T Hc[5], Hm[5], Hp[5], hh[5], HF[5];
+#pragma unroll
+          for (int q = 0; q < 5; ++q) { Hc[q] = u_at(q, hy, hx); Hm[q] = u_at(q, hy - 1, hx); Hp[q] = u_at(q, hy + 1, hx); }
+          hh[0] = Hc[0];
+#pragma unroll
+          for (int q = 1; q < 5; ++q) hh[q] = (T)0.5 * (Hc[q] + l_at(q - 1, hy, hx));
+          T hxi = l_at(5, hy, hx);
+          if (side) {
+            flux_parts<T, 2>(P, 1, Hc, Hm, Hp, hh, hxi, HF, HF);
+#pragma unroll
+            for (int q = 0; q < 5; ++q) sE[((q + 5) * (TY + 2) + TY + 1) * TX + hx] = HF[q];
+          } else {
+            flux_parts<T, 1>(P, 1, Hc, Hm, Hp, hh, hxi, HF, HF);
+#pragma unroll
+            for (int q = 0; q < 5; ++q) sE[(q * (TY + 2) + 0) * TX + hx] = HF[q];
+          }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 5; ++q)
+          a[q] += sE[((q + 5) * (TY + 2) + ty + 2) * TX + tx] - sE[(q * (TY + 2) + ty) * TX + tx];
+      }
+      // z: own parts of plane p, FP of plane p-1; FM of plane p+1 is added when it is known
+#pragma unroll
+      for (int q = 0; q < 5; ++q) {
+        acc[q] = a[q] + ((FPz[q] - FMz[q]) - FPzp[q]);
+        Utp[q] = q == 0 ? U0[0] : l_at(q - 1, ty, tx);
+      }
+    }
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { FPzp[q] = FPz[q]; Um[q] = U0[q]; }
+    __syncthreads();                                   // everyone is done with stage s and with sE
+    if (tid == 0 && p + 2 <= z1) issue(p + 2, s);
+  }
+  block_max_to_global<T>(smax, smax_out);
+}
+
+}  // namespace cspt

@@ -19,58 +19,6 @@
 
 namespace cspt {
 
-// 1/sqrt(s) and sqrt(s) for s > 0, accurate to rounding level for the type.
-template <class T> struct Fast;
-template <> struct Fast<double> {
-  // MUFU.RSQ64H seed (about 2^-20 relative) + one third-order step: y = y0 (1 + e/2 + 3e^2/8),
-  // e = 1 - s y0^2;  sqrt(s) = s y0 (1 + e/2 + 3e^2/8).  Six FP64 instructions, no branches.
-  static __device__ __forceinline__ void rsqrt_sqrt(double s, double& y, double& t) {
-    double y0;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(s));
-    double t0 = s * y0;
-    double e = fma(-t0, y0, 1.0);
-    double ce = fma(0.375, e, 0.5) * e;
-    y = fma(y0, ce, y0);
-    t = fma(t0, ce, t0);
-  }
-  // 1/x for normal x > 0: MUFU.RCP64H seed + one third-order step, y = y0 (1 + e + e^2), e = 1 - x y0
-  static __device__ __forceinline__ double rcp(double x) {
-    double y0;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y0) : "d"(x));
-    double e = fma(-x, y0, 1.0);
-    return fma(y0, fma(e, e, e), y0);
-  }
-  // sqrt(x) for x >= 0; values below 1e-280 (phi < 1e-140) are flushed to 0
-  static __device__ __forceinline__ double sqrt0(double x) {
-    double y, t;
-    rsqrt_sqrt(x, y, t);
-    return x > 1e-280 ? t : 0.0;
-  }
-  // comparisons of a positive double with 1 and 4 on the high word (integer pipe)
-  static __device__ __forceinline__ bool lt1(double s) { return __double2hiint(s) < 0x3FF00000; }
-  static __device__ __forceinline__ bool lt4(double s) { return __double2hiint(s) < 0x40100000; }
-  static __device__ __forceinline__ double tiny() { return 1e-300; }
-};
-template <> struct Fast<float> {
-  static __device__ __forceinline__ void rsqrt_sqrt(float s, float& y, float& t) {
-    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(s));
-    t = s * y;
-  }
-  static __device__ __forceinline__ float rcp(float x) {
-    float y;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-  }
-  static __device__ __forceinline__ float sqrt0(float x) {
-    float y;
-    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
-    return y;
-  }
-  static __device__ __forceinline__ bool lt1(float s) { return s < 1.0f; }
-  static __device__ __forceinline__ bool lt4(float s) { return s < 4.0f; }
-  static __device__ __forceinline__ float tiny() { return 1e-30f; }
-};
-
 // Field order of the star group (slot S_ST): what the predictor hands to the corrector.
 enum StarField { ST_PHI = 0, ST_U, ST_V, ST_W, ST_EX, ST_EY, ST_EZ, ST_E, ST_COUNT };
 
