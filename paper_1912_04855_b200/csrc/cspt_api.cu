@@ -354,8 +354,8 @@ int step_cfl_t(cspt_ctx* c, double cfl, double* out) {
 }
 
 // dense staging arrays for the *_host entry points live in the (dead between steps)
-// intermediate slots S_PR.. (12 padded slots >= 6 dense arrays)
-template <class T> T* staging(cspt_ctx* c, int f) { return field<T>(c, S_PR + f); }
+// star-group slots S_ST.. (8 padded slots >= 6 dense arrays)
+template <class T> T* staging(cspt_ctx* c, int f) { return field<T>(c, S_ST + f); }
 
 }  // namespace
 

@@ -50,9 +50,9 @@ enum Slot {
   S_F = 10,        // f = -D[psi]                                (3)
   S_UT = 13,       // U~: mx, my, mz, E  (rho~ = rho^n, G2)      (4)
   S_XI = 17,       // xi^{n+1}                                   (3)
-  S_PR = 20,       // scratch (dense staging of the *_host entry points)  (4)
-  S_ST = 24,       // star group: phi*, u*, v*, w*, eta* (3), E* (8)
-  S_COUNT = 32
+  S_ST = 20,       // star group: phi*, u*, v*, w*, eta* (3), E* (8); between steps: dense staging
+                   // arrays of the *_host entry points
+  S_COUNT = 28
 };
 
 template <class T> struct Real;

@@ -1,0 +1,154 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times
+(`cspt_step_cfl`, device-resident dt): sampled windows the oracle can afford (SURVEY.md
+section 8(d)).
+
+One full step reaches +-3 cells (readings G16), so after S steps the state inside a window
+depends only on the initial data within 3*S cells of it.  The GPU runs the whole grid S
+steps with its own CFL time steps; for every window the oracle is started from the same
+seeded initial data on the window padded by 3*S cells (regenerated from global cell
+indices), is fed the GPU's dt sequence, and the window cores are compared element by
+element.  Sides of the padded window that lie on the physical boundary use the real
+boundary rule; the other sides are arbitrary (OUTFLOW), their influence never reaches the
+core.  The error is normwise per conserved field (G21), measured against max|field| over
+the whole GPU grid (a window may be all vacuum).
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle_util import make_oracle
+from paper_1912_04855_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-11
+TOL32 = 1e-4
+REACH = 3          # cells per step
+
+
+@pytest.fixture(scope="module")
+def cspt():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1912_04855_b200 import build, cspt as mod
+    build.build()
+    mod.lib()
+    return mod
+
+
+def device_fields(w, device):
+    """The six input fields as device tensors, generated slab by slab (no full-size host copy)."""
+    import torch
+    from concurrent.futures import ThreadPoolExecutor
+    tdt = torch.float64 if w.dtype == "f64" else torch.float32
+    out = [torch.empty((w.nz, w.ny, w.nx), dtype=tdt, device=device) for _ in range(6)]
+    slab = max(1, min(w.nz, (1 << 23) // max(1, w.nx * w.ny)))
+    starts = list(range(0, w.nz, slab))
+    with ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1)) as ex:
+        for k0, f in zip(starts, ex.map(lambda k0: w.fields_slab(k0, min(w.nz, k0 + slab)), starts)):
+            for t, a in zip(out, f):
+                t[k0:k0 + a.shape[0]].copy_(torch.from_numpy(np.ascontiguousarray(a)))
+    return out
+
+
+def window_box(w, lo, size, pad):
+    """Per axis: (core start, core stop, padded start, padded stop, bc_lo, bc_hi) with the padded
+    range clipped at non-periodic physical faces (where the real boundary kind applies)."""
+    n = (w.nx, w.ny, w.nz)
+    box = []
+    for d in range(3):
+        c0, c1 = lo[d], min(n[d], lo[d] + size[d])
+        p0, p1 = c0 - pad, c1 + pad
+        blo = bhi = wl.OUTFLOW
+        periodic = w.bc[2 * d] == wl.PERIODIC
+        if periodic and n[d] <= (c1 - c0) + 2 * pad:      # the window wraps onto itself: take the whole axis
+            p0, p1, blo, bhi = 0, n[d], wl.PERIODIC, wl.PERIODIC
+        elif not periodic:
+            if p0 <= 0:
+                p0, blo = 0, w.bc[2 * d]
+            if p1 >= n[d]:
+                p1, bhi = n[d], w.bc[2 * d + 1]
+        box.append((c0, c1, p0, p1, blo, bhi))
+    return box
+
+
+def check_windows(cspt, oracle_mod, w, windows, steps, tol, size=(48, 48, 48)):
+    import torch
+    dev = torch.device("cuda", torch.cuda.current_device())
+    s = cspt.Solver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, cspt.F64 if w.dtype == "f64" else cspt.F32)
+    f = device_fields(w, dev)
+    s.set_state(*f)
+    del f
+    torch.cuda.empty_cache()
+    dts = [s.step_cfl(w.cfl, want_dt=True) for _ in range(steps)]
+    assert all(np.isfinite(dts)) and min(dts) > 0
+    got = s.get_conserved()
+    scale = [float(t.abs().max().item()) for t in got]
+    mscale = (scale[0] * scale[4]) ** 0.5
+    for q in (1, 2, 3):                      # a momentum component that vanishes identically (G21)
+        if scale[q] < 1e-6 * mscale:
+            scale[q] = mscale
+    pad = REACH * steps
+    worst = 0.0
+    for lo in windows:
+        box = window_box(w, lo, size, pad)
+        idx = [np.arange(b[2], b[3]) for b in box]
+        bc = [box[0][4], box[0][5], box[1][4], box[1][5], box[2][4], box[2][5]]
+        fw = w.fields(idx[0], idx[1], idx[2])
+        ww = wl.Workload("window", len(idx[0]), len(idx[1]), len(idx[2]), w.h, w.gamma, bc, w.origin, w.cfl, steps,
+                         w.dtype, None)
+        o = make_oracle(oracle_mod, ww, dtype="f64")
+        o.set_state(*[np.asarray(a, dtype=np.float64) for a in fw])
+        for dt in dts:
+            o.step(dt)
+        ref = o.get_conserved()
+        o.close()
+        core = tuple(slice(box[d][0] - box[d][2], box[d][1] - box[d][2]) for d in (2, 1, 0))
+        gsl = tuple(slice(box[d][0], box[d][1]) for d in (2, 1, 0))
+        for q in range(5):
+            a = got[q][gsl].double().cpu().numpy()
+            err = float(np.max(np.abs(a - ref[q][core]))) / scale[q]
+            worst = max(worst, err)
+            assert err < tol, (w.name, lo, q, err)
+    s.close()
+    return worst
+
+
+def corner_and_centre_windows(w, size=48):
+    n = (w.nx, w.ny, w.nz)
+    c = tuple(n[d] // 2 - size // 2 for d in range(3))
+    return [c, (0, 0, 0), (n[0] - size, n[1] // 3, 0), (n[0] // 5, n[1] - size, n[2] - size)]
+
+
+def test_cfg2_sedov_128_full_grid(cspt, oracle_mod):
+    """128^3 is small enough for the oracle: one window = the whole grid."""
+    w = wl.sedov()
+    check_windows(cspt, oracle_mod, w, [(0, 0, 0)], 5, TOL64, size=(128, 128, 128))
+
+
+def test_cfg3_well_256_windows(cspt, oracle_mod):
+    w = wl.well()
+    wins = corner_and_centre_windows(w) + [(0, 100, 100)]          # inflow face
+    check_windows(cspt, oracle_mod, w, wins, 6, TOL64)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_cfg4_turbulence_512_windows(cspt, oracle_mod, dtype):
+    w = wl.turbulence(dtype=dtype)
+    check_windows(cspt, oracle_mod, w, corner_and_centre_windows(w), 6, TOL64 if dtype == "f64" else TOL32)
+
+
+def test_cfg5_disk_1024_windows(cspt, oracle_mod):
+    import torch
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    if free < 156 * 2 ** 30:
+        pytest.skip("needs about 150 GiB of free device memory (workspace 124 GB + inputs 26 GB)")
+    w = wl.disk()
+    n, sz = w.nx, 48
+    wins = [(n // 2 - sz // 2,) * 3,                    # disk centre
+            (n // 2 + 200, n // 2 - sz // 2, n // 2 - 10),  # in the disk, off centre
+            (n // 2 + int(0.4 * n) - sz // 2, n // 2, n // 2 - sz // 2),   # the gas-vacuum edge R = 0.4 L
+            (0, 0, 0)]                                   # vacuum corner with outflow faces
+    check_windows(cspt, oracle_mod, w, wins, 5, TOL32)
