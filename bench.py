@@ -44,6 +44,12 @@ KERNEL_WORDS = {
 }
 
 
+# Algorithmic floating-point operations per cell (FMA = 2) of the ALU-bound kernels:
+# corrector = 26 neighbours x (3 sub, 3 FMA, 6 for 1/sqrt and sqrt, 3 for the spline, 1 mul, 3 FMA, 4 for the
+# energy term = 23 instructions, 17 of them FMA -> 40 flop) + about 60 flop for Eq. (6).
+KERNEL_FLOPS = {"corrector": 26 * 40 + 60}
+
+
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -236,6 +242,25 @@ def run_reference(args):
 
 
 # ---------------------------------------------------------------------------------------
+# N > 1: "replicas only" -- no data-path collective, only the timing reduction
+# ---------------------------------------------------------------------------------------
+def max_over_ranks(ms, world, device):
+    """Device time of the slowest rank (all ranks get it)."""
+    if world == 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(cells_per_rank, steps, world, tmax_ms):
+    """Whole-job Mcell-updates/s: the cells all ranks advanced, over the slowest rank's time."""
+    return world * cells_per_rank * steps / (tmax_ms * 1e-3) / 1e6
+
+
+# ---------------------------------------------------------------------------------------
 # the CUDA path
 # ---------------------------------------------------------------------------------------
 def run_cspt(args):
@@ -290,12 +315,8 @@ def run_cspt(args):
     prof = s.profile_read()
     s.profile_enable(False)
     launches = s.launch_count() - l0
-    tmax = ms
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        tmax = float(t.item())
-    value = world * w.cells * args.steps / (tmax * 1e-3) / 1e6
+    tmax = max_over_ranks(ms, world, "cuda")
+    value = job_value(w.cells, args.steps, world, tmax)
 
     # the state must still be sane (a blown-up run would time NaN arithmetic)
     rho = s.get_conserved()[0]
@@ -317,11 +338,8 @@ def run_cspt(args):
     f1.record(s.stream)
     barrier()
     ems = f0.elapsed_time(f1)
-    if world > 1:
-        t = torch.tensor([ems], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ems = float(t.item())
-    e2e = {"value": world * w.cells * n_e2e / (ems * 1e-3) / 1e6, "unit": UNIT,
+    ems = max_over_ranks(ems, world, "cuda")
+    e2e = {"value": job_value(w.cells, n_e2e, world, ems), "unit": UNIT,
            "h2d_bytes_per_step": 6 * w.cells * esz, "d2h_bytes_per_step": 5 * w.cells * esz, "steps": n_e2e,
            "what": "cspt_set_state_host + cspt_step_cfl + cspt_get_conserved_host per step, pinned host buffers"}
 
@@ -339,9 +357,30 @@ def run_cspt(args):
     words = KERNEL_WORDS.get(dom, MIN_WORDS_PER_CELL)
     dom_bytes = words * esz * w.cells
     ach = dom_bytes / (dom_ms * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": None, "peak_source": peak_src, "algorithmic_bytes_per_launch": dom_bytes,
-                "kernel_ms": dom_ms, "share_of_step": (prof[dom][0] / args.steps) / step_ms}
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            traffic = json.load(fh).get("%s %dx%dx%d %s" % (w.name, w.nx, w.ny, w.nz, w.dtype), {}).get(dom)
+    except Exception:
+        traffic = None
+    hbm = {"achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": peak_src,
+           "algorithmic_bytes_per_launch": dom_bytes}
+    if dom in KERNEL_FLOPS:
+        # the corrector is bound by the plain FP64 / FP32 pipe: algorithmic flops per cell
+        # (FMA = 2) over the launch time, against lanes x 2 flop x SMs x max SM clock
+        lanes = 64 if w.dtype == "f64" else 128
+        apeak = 148 * lanes * 2 * 1.965e9 / 1e12
+        aach = KERNEL_FLOPS[dom] * w.cells / (dom_ms * 1e-3) / 1e12
+        roofline = {"bound": "alu", "kernel": dom, "achieved": aach, "peak": apeak, "unit": "TFLOP/s",
+                    "frac": aach / apeak, "traffic": traffic,
+                    "peak_source": "derived: 148 SMs x %d %s lanes x 2 flop x 1965 MHz (DESIGN.md section 7; "
+                                   "measured 63.4 DFMA / 120.9 FFMA per clock per SM, profiles/r1a_launches_baseline.md)"
+                                   % (lanes, w.dtype),
+                    "algorithmic_flops_per_cell": KERNEL_FLOPS[dom], "kernel_ms": dom_ms,
+                    "share_of_step": (prof[dom][0] / args.steps) / step_ms, "hbm": hbm}
+    else:
+        roofline = dict(hbm, bound="hbm", kernel=dom, traffic=traffic, kernel_ms=dom_ms,
+                        share_of_step=(prof[dom][0] / args.steps) / step_ms)
     step_ach = MIN_WORDS_PER_CELL * esz * w.cells / (step_ms * 1e-3) / 1e9
     step_hbm = {"bytes_per_cell_update": MIN_WORDS_PER_CELL * esz, "achieved_gbs": step_ach, "frac_of_measured": step_ach / peak,
                 "frac_of_nominal_8TBs": step_ach / 8000.0}
