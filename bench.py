@@ -395,7 +395,7 @@ def run_cspt(args):
     }
 
     if not args.no_cpu_baseline and world == 1:
-        n_s = min(160, max(w.nx, w.ny, w.nz)) if args.workload != "sod" else None
+        n_s = min(384, max(w.nx, w.ny, w.nz)) if args.workload != "sod" else None
         ws, times, cores = oracle_sample(args, w, 3, 0, n_s)
         tot = sum(times)
         line["cpu_baseline"] = {"value": ws.cells * len(times) / tot / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
