@@ -74,24 +74,15 @@ k_euler_block(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ 
     for (int q = 0; q < 5; ++q) { Um[q] = inside ? U[c + q * fs] : (T)0; FPzp[q] = 0; acc[q] = 0; Utp[q] = 0; }
   }
 
-  // own column of plane p+1 comes straight from global memory (it becomes a TMA box one iteration
-  // later); it is requested a full iteration ahead so that its latency is hidden
-  const long long c_col = L.idx(inside ? i : 0, inside ? j : 0, 0), szp = L.sz();
-  T Unext[5];
-#pragma unroll
-  for (int q = 0; q < 5; ++q) Unext[q] = __ldg(U + c_col + (long long)z0 * szp + q * fs);
+  // The z+ neighbour of the own column (plane p+1) is read from the OTHER ring stage, which plane p+1 is
+  // landing in while plane p is processed: the z parts are therefore formed last in the iteration, after
+  // waiting for that stage (a global load here would share a scoreboard with the shared-memory loads
+  // and expose the DRAM latency every plane).
   uint32_t phase = 0;        // bit s: parity to wait for on stage s
+  mbar_wait(&bar[0], 0u);
+  phase ^= 1u;
   for (int p = z0 - 1; p <= z1; ++p) {
     const int s = (p - (z0 - 1)) & 1;
-    T Up[5];
-#pragma unroll
-    for (int q = 0; q < 5; ++q) Up[q] = Unext[q];
-    if (p < z1) {
-#pragma unroll
-      for (int q = 0; q < 5; ++q) Unext[q] = __ldg(U + c_col + (long long)(p + 2) * szp + q * fs);
-    }
-    mbar_wait(&bar[s], (phase >> s) & 1u);
-    phase ^= 1u << s;
     const T* sU = (const T*)(sm + S::OFF_U + s * S::U_STAGE);
     const T* sL = (const T*)(sm + S::OFF_L + s * S::L_STAGE);
     auto u_at = [&](int q, int y, int x) { return sU[(q * S::UY + (y + 2)) * S::BX + (x + S::HX)]; };   // tile coords
@@ -104,26 +95,9 @@ k_euler_block(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ 
 #pragma unroll
     for (int q = 1; q < 5; ++q) hf[q] = (T)0.5 * (U0[q] + l_at(q - 1, ty, tx));
 
-    // z axis: both parts of plane p
-    T FPz[5], FMz[5];
-    flux_parts<T, 3>(P, 2, U0, Um, Up, hf, l_at(6, ty, tx), FPz, FMz);
-
-    // finish cell p-1 (SUE, Eq. (4))
-    if (p - 1 >= z0) {
-      T un[5];
-#pragma unroll
-      for (int q = 0; q < 5; ++q) un[q] = Utp[q] - lam * (acc[q] + FMz[q]);
-      if (inside) {
-        long long c = L.idx(i, j, p - 1);
-#pragma unroll
-        for (int q = 0; q < 5; ++q) UN[c + q * fs] = un[q];
-        T sp = cell_speed_exact<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
-        smax = sp > smax ? sp : smax;
-      }
-    }
-
-    if (p >= z0 && p < z1) {
-      T a[5];
+    const bool active = p >= z0 && p < z1;
+    T a[5] = {0, 0, 0, 0, 0};
+    if (active) {
       // ---- x axis -------------------------------------------------------------
       {
         T Ux0[5], Ux1[5], FP[5], FM[5];
@@ -200,6 +174,31 @@ k_euler_block(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ 
         for (int q = 0; q < 5; ++q)
           a[q] += sE[((q + 5) * (TY + 2) + ty + 2) * TX + tx] - sE[(q * (TY + 2) + ty) * TX + tx];
       }
+    }
+    // z axis: both parts of plane p; U^n of plane p+1 from the other stage
+    T Up[5], FPz[5], FMz[5];
+    mbar_wait(&bar[s ^ 1], (phase >> (s ^ 1)) & 1u);
+    phase ^= 1u << (s ^ 1);
+    {
+      const T* sU1 = (const T*)(sm + S::OFF_U + (s ^ 1) * S::U_STAGE);
+#pragma unroll
+      for (int q = 0; q < 5; ++q) Up[q] = sU1[(q * S::UY + (ty + 2)) * S::BX + (tx + S::HX)];
+    }
+    flux_parts<T, 3>(P, 2, U0, Um, Up, hf, l_at(6, ty, tx), FPz, FMz);
+    // finish cell p-1 (SUE, Eq. (4))
+    if (p - 1 >= z0) {
+      T un[5];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) un[q] = Utp[q] - lam * (acc[q] + FMz[q]);
+      if (inside) {
+        long long c = L.idx(i, j, p - 1);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) UN[c + q * fs] = un[q];
+        T sp = cell_speed_exact<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
+        smax = sp > smax ? sp : smax;
+      }
+    }
+    if (active) {
       // z: own parts of plane p, FP of plane p-1; FM of plane p+1 is added when it is known
 #pragma unroll
       for (int q = 0; q < 5; ++q) {
@@ -210,7 +209,7 @@ k_euler_block(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ 
 #pragma unroll
     for (int q = 0; q < 5; ++q) { FPzp[q] = FPz[q]; Um[q] = U0[q]; }
     __syncthreads();                                   // everyone is done with stage s and with sE
-    if (tid == 0 && p + 2 <= z1) issue(p + 2, s);
+    if (tid == 0 && p + 2 <= z1 + 1) issue(p + 2, s);
   }
   block_max_to_global<T>(smax, smax_out);
 }
