@@ -6,7 +6,6 @@
 
 #include "cspt_step.cuh"
 #include "cspt_euler.cuh"
-#include "cspt_euler_block.cuh"
 #include "cspt_lagrange.cuh"
 
 using namespace cspt;
@@ -196,8 +195,7 @@ int compute_dt_t(cspt_ctx* c, double cfl, double* out) {
   return CSPT_OK;
 }
 
-// Euler-stage tile: one warp per row plus two halo-row warps; 6 rows in fp64 (8 warps, 128 registers
-// per thread at 2 CTAs per SM), 8 rows in fp32
+// Euler-stage tile (threads = cells of one plane of the column)
 constexpr int ETX = 32;
 template <class T> struct EulerTile { static constexpr int TY = 8; };
 
@@ -255,12 +253,8 @@ bool make_maps(cspt_ctx* c) {
                               S::BX, S::UY, 5);
   ok = ok && make_field_map(&c->mapL, field<T>(c, S_UT), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 7, S::BX, S::LY, 7);
   if (ok) {
-    // both layouts of the stage read the same boxes (TX x TY tile, halo 2 / 1)
-    static_assert(EulerSmemB<T, ETX, ETY>::BX == S::BX && EulerSmemB<T, ETX, ETY>::UY == S::UY, "same TMA boxes");
     ok = cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
-             cudaSuccess &&
-         cudaFuncSetAttribute(k_euler_block<T, ETX, ETY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              EulerSmemB<T, ETX, ETY>::BYTES) == cudaSuccess;
+         cudaSuccess;
   }
   ok = ok && corr_dispatch<T>(c, nullptr, nullptr);
   return ok;
@@ -297,14 +291,8 @@ void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
   dim3 grid(gx, gy, (L.nz + zc - 1) / zc);
   DevScalars<T>* sc = scalars<T>(c);
   int ps_ = prof_open(c, K_EULER);
-  if (c->euler_variant == 1) {
-    typedef EulerSmemB<T, ETX, ETY> SB;
-    k_euler_block<T, ETX, ETY><<<grid, ETX * ETY, SB::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN,
-                                                                          &sc->smax_bits, zc);
-  } else {
-    k_euler_stream<T, ETX, ETY><<<grid, S::THREADS, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN,
-                                                                           &sc->smax_bits, zc);
-  }
+  k_euler_stream<T, ETX, ETY><<<grid, ETX * ETY, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN,
+                                                                        &sc->smax_bits, zc);
   prof_close(c, ps_);
   c->launches++;
 }
@@ -403,8 +391,7 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->have_maps = dtype == CSPT_F64 ? make_maps<double>(c) : make_maps<float>(c);
   if (!c->have_maps) { (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }
   c->legacy_euler = getenv("CSPT_LEGACY_EULER") != nullptr;
-  // layout of the Euler stage: block layout in fp64, halo-warp layout in fp32 (measured on B200); tuning switch
-  c->euler_variant = getenv("CSPT_EULER_VARIANT") ? atoi(getenv("CSPT_EULER_VARIANT")) : (dtype == CSPT_F64 ? 1 : 0);
+
   *out = c;
   return CSPT_OK;
 }

@@ -112,7 +112,6 @@ struct cspt_ctx {
   CUtensorMap mapU[2], mapL, mapS;
   bool have_maps;
   int corr_variant;         // tuning switch (env CSPT_CORR_VARIANT): corrector tile variant
-  int euler_variant;        // 0: halo-warp layout (cspt_euler.cuh), 1: block layout (cspt_euler_block.cuh)
   bool legacy_euler;        // debug switch (env CSPT_LEGACY_EULER): first, unfused Euler kernel
   // per-kernel device timing (cspt_profile_*): event pairs recorded around each launch
   bool prof_on;

@@ -2,16 +2,16 @@
 // PAPER.md:45-50, :70-78, :112-113; readings G9-G14, with the CFL signal speed of U^{n+1}
 // (G15) as epilogue.
 //
-// One CTA owns a TX x TY column of cells and streams along z (2.5-D): per plane one TMA box
-// of U^n (halo 2 in x/y) and one of (U~, xi) (halo 1) land in a 2-stage shared-memory ring.
-// Per cell and axis the two one-sided flux parts
+// One CTA owns a TX x TY column of cells (one thread per cell of a plane) and streams along z
+// (2.5-D): per plane one TMA box of U^n (halo 2 in x/y) and one of (U~, xi) (halo 1) land in a
+// 2-stage shared-memory ring.  Per cell and axis the two one-sided flux parts
 //     FP_i = max(u^L_i,0) U^L_i   (leaves through the + face),   FM_i = min(u^R_i,0) U^R_i   (through the - face)
-// are computed ONCE (F_{i+1/2} = FP_i + FM_{i+1}).  The CTA has TY + 2 warps: warp r+1 owns row r of the
-// tile (TX = 32 cells = its lanes); the two extra warps own the halo rows -1 and TY, of which only the
-// y parts are needed, and use their spare time for the x parts of the halo columns -1 and TX.  Parts
-// travel to the x neighbours by warp shuffles, to the y neighbours through shared memory (one
-// barrier), and along z in registers: the thread keeps FP of the previous plane and finishes cell
-// p-1 when FM of plane p is known.
+// are computed ONCE (F_{i+1/2} = FP_i + FM_{i+1}) and handed to the x and y neighbours through
+// shared memory (the parts of the halo columns / rows are computed by the first / the last warps);
+// along z the thread keeps FP of the previous plane in registers and finishes cell p-1 when FM of
+// plane p is known.  The z+ neighbour U^n(p+1) of the own column is read from the other ring stage.
+// (A second layout with one warp per row, two halo-row warps and x exchange by warp shuffles was
+// measured slower in both precisions and removed: 6.1 / 4.2 ms against 5.4 / 3.3 ms at 512^3.)
 #pragma once
 #include "cspt_kernels.cuh"
 #include "cspt_tma.cuh"
@@ -54,7 +54,6 @@ __device__ __forceinline__ void flux_parts(const Params<T>& P, int d, const T* U
 
 template <class T, int TX, int TY>
 struct EulerSmem {
-  static_assert(TX == 32, "a warp owns one row of the tile");
   // x halo of the boxes: 2 cells are needed; 16 bytes' worth are loaded so that every box row starts
   // on a 16-byte boundary in global memory (an 8-byte-aligned fp32 start raised "illegal instruction")
   static constexpr int HX = 16 / (int)sizeof(T) < 2 ? 2 : 16 / (int)sizeof(T);
@@ -64,36 +63,29 @@ struct EulerSmem {
   static constexpr int L_ELEMS = 7 * LY * BX;
   static constexpr int U_STAGE = (U_ELEMS * (int)sizeof(T) + 127) / 128 * 128;    // bytes
   static constexpr int L_STAGE = (L_ELEMS * (int)sizeof(T) + 127) / 128 * 128;
-  // y exchange: FP of rows -1..TY-1 and FM of rows 0..TY;  x halo columns: FP of x = -1, FM of x = TX
-  static constexpr int EY_ELEMS = 10 * (TY + 1) * TX;
-  static constexpr int EX_ELEMS = 10 * TY;
+  static constexpr int EX_ELEMS = 10 * (TX + 2) * (TY + 2);                       // exchange buffer (x, then y)
   static constexpr int OFF_U = 0;
   static constexpr int OFF_L = OFF_U + 2 * U_STAGE;
-  static constexpr int OFF_EY = OFF_L + 2 * L_STAGE;
-  static constexpr int OFF_EX = OFF_EY + (EY_ELEMS * (int)sizeof(T) + 127) / 128 * 128;
-  static constexpr int OFF_BAR = OFF_EX + (EX_ELEMS * (int)sizeof(T) + 127) / 128 * 128;
-  static constexpr int BYTES = OFF_BAR + 64;
-  static constexpr int THREADS = TX * (TY + 2);
+  static constexpr int OFF_E = OFF_L + 2 * L_STAGE;
+  static constexpr int OFF_BAR = OFF_E + (EX_ELEMS * (int)sizeof(T) + 127) / 128 * 128;
+  static constexpr int BYTES = OFF_BAR + 64 + 128;  // + slack for the 128-byte alignment of the base
 };
 
 template <class T, int TX, int TY>
-__global__ void __launch_bounds__(TX*(TY + 2), 2)
+__global__ void __launch_bounds__(TX* TY, 2)
 k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL, Params<T> P,
                const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, T* __restrict__ UN,
                typename Real<T>::bits_t* __restrict__ smax_out, int zchunk) {
   typedef EulerSmem<T, TX, TY> S;
   extern __shared__ __align__(128) unsigned char sm[];
   uint64_t* bar = (uint64_t*)(sm + S::OFF_BAR);
-  T* sEY = (T*)(sm + S::OFF_EY);
-  T* sEX = (T*)(sm + S::OFF_EX);
+  T* sE = (T*)(sm + S::OFF_E);
   const Layout& L = P.L;
-  const int tid = threadIdx.x, tx = tid % TX;
-  const int ty = tid / TX - 1;                       // row of the tile: -1 and TY are the halo rows
-  const bool main_row = ty >= 0 && ty < TY;
+  const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
   const int i0 = blockIdx.x * TX, j0 = blockIdx.y * TY;
   const int z0 = blockIdx.z * zchunk, z1 = min(L.nz, z0 + zchunk);
   const int i = i0 + tx, j = j0 + ty;
-  const bool inside = main_row && i < L.nx && j < L.ny;
+  const bool inside = i < L.nx && j < L.ny;
   const long long fs = L.fstride;
   constexpr uint32_t TX_BYTES = (uint32_t)((S::U_ELEMS + S::L_ELEMS) * sizeof(T));
 
@@ -119,143 +111,149 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
   const T lam = dt * P.inv_h;
   T Um[5], FPzp[5], acc[5], Utp[5];
   T smax = 0;
-  // own column of planes z0-2 (z slope of plane z0-1) and, one iteration ahead of its use, p+1: straight
-  // from global memory (plane p+1 becomes a TMA box one iteration later)
-  const long long c_col = L.idx(inside ? i : 0, inside ? j : 0, 0), szp = L.sz();
-  T Unext[5];
+  // U^n of plane z0-2 (own column) for the z slope of plane z0-1
+  {
+    long long c = L.idx(inside ? i : 0, inside ? j : 0, z0 - 2);
 #pragma unroll
-  for (int q = 0; q < 5; ++q) {
-    Um[q] = main_row ? __ldg(U + c_col + (long long)(z0 - 2) * szp + q * fs) : (T)0;
-    Unext[q] = main_row ? __ldg(U + c_col + (long long)z0 * szp + q * fs) : (T)0;
-    FPzp[q] = 0; acc[q] = 0; Utp[q] = 0;
+    for (int q = 0; q < 5; ++q) { Um[q] = inside ? U[c + q * fs] : (T)0; FPzp[q] = 0; acc[q] = 0; Utp[q] = 0; }
   }
 
+  // The z+ neighbour of the own column (plane p+1) is read from the OTHER ring stage, which plane p+1 is
+  // landing in while plane p is processed: the z parts are therefore formed last in the iteration, after
+  // waiting for that stage (a global load here would share a scoreboard with the shared-memory loads
+  // and expose the DRAM latency every plane).
   uint32_t phase = 0;        // bit s: parity to wait for on stage s
+  mbar_wait(&bar[0], 0u);
+  phase ^= 1u;
   for (int p = z0 - 1; p <= z1; ++p) {
-    const int K = (p - (z0 - 1)) & 1;
-    T Up[5];
-#pragma unroll
-    for (int q = 0; q < 5; ++q) Up[q] = Unext[q];
-    if (p < z1 && main_row) {
-#pragma unroll
-      for (int q = 0; q < 5; ++q) Unext[q] = __ldg(U + c_col + (long long)(p + 2) * szp + q * fs);
-    }
-    mbar_wait(&bar[K], (phase >> K) & 1u);
-    phase ^= 1u << K;
-    const T* sU = (const T*)(sm + S::OFF_U + K * S::U_STAGE);
-    const T* sL = (const T*)(sm + S::OFF_L + K * S::L_STAGE);
+    const int s = (p - (z0 - 1)) & 1;
+    const T* sU = (const T*)(sm + S::OFF_U + s * S::U_STAGE);
+    const T* sL = (const T*)(sm + S::OFF_L + s * S::L_STAGE);
     auto u_at = [&](int q, int y, int x) { return sU[(q * S::UY + (y + 2)) * S::BX + (x + S::HX)]; };   // tile coords
     auto l_at = [&](int q, int y, int x) { return sL[(q * S::LY + (y + 1)) * S::BX + (x + S::HX)]; };
-    // U^n, its two neighbours along axis d and U^{n+1/2} (G10; rho~ = rho^n, G2) of tile cell (x, y)
-    auto gather = [&](int d, int y, int x, T* Uc, T* Ua, T* Ub, T* hf) {
-      const int ax = d == 0, ay = d == 1;
-#pragma unroll
-      for (int q = 0; q < 5; ++q) { Uc[q] = u_at(q, y, x); Ua[q] = u_at(q, y - ay, x - ax); Ub[q] = u_at(q, y + ay, x + ax); }
-      hf[0] = Uc[0];
-#pragma unroll
-      for (int q = 1; q < 5; ++q) hf[q] = (T)0.5 * (Uc[q] + l_at(q - 1, y, x));
-    };
-    const bool active = p >= z0 && p < z1;
 
-    if (main_row) {
-      T U0[5], hf[5], FPz[5], FMz[5];
+    T U0[5], hf[5];
 #pragma unroll
-      for (int q = 0; q < 5; ++q) U0[q] = u_at(q, ty, tx);
-      hf[0] = U0[0];
+    for (int q = 0; q < 5; ++q) U0[q] = u_at(q, ty, tx);
+    hf[0] = U0[0];                                              // rho~ = rho^n (G2)
 #pragma unroll
-      for (int q = 1; q < 5; ++q) hf[q] = (T)0.5 * (U0[q] + l_at(q - 1, ty, tx));
-      // z axis: both parts of plane p
-      flux_parts<T, 3>(P, 2, U0, Um, Up, hf, l_at(6, ty, tx), FPz, FMz);
-      // finish cell p-1 (SUE, Eq. (4))
-      if (p - 1 >= z0) {
-        T un[5];
+    for (int q = 1; q < 5; ++q) hf[q] = (T)0.5 * (U0[q] + l_at(q - 1, ty, tx));
+
+    const bool active = p >= z0 && p < z1;
+    T a[5] = {0, 0, 0, 0, 0};
+    if (active) {
+      // ---- x axis -------------------------------------------------------------
+      {
+        T Ux0[5], Ux1[5], FP[5], FM[5];
 #pragma unroll
-        for (int q = 0; q < 5; ++q) un[q] = Utp[q] - lam * (acc[q] + FMz[q]);
-        if (inside) {
-          long long c = L.idx(i, j, p - 1);
-#pragma unroll
-          for (int q = 0; q < 5; ++q) UN[c + q * fs] = un[q];
-          T sp = cell_speed_exact<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
-          smax = sp > smax ? sp : smax;
-        }
-      }
-      if (active) {
-        T Ua[5], Ub[5], FP[5], FM[5];
-        // z: own parts of plane p, FP of plane p-1; FM of plane p+1 is added when it is known
+        for (int q = 0; q < 5; ++q) { Ux0[q] = u_at(q, ty, tx - 1); Ux1[q] = u_at(q, ty, tx + 1); }
+        flux_parts<T, 3>(P, 0, U0, Ux0, Ux1, hf, l_at(4, ty, tx), FP, FM);
+        // exchange layout: [q][ty][tx+1], FP in 0..4, FM in 5..9, row pitch TX+2
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
-          acc[q] = (FPz[q] - FMz[q]) - FPzp[q];
-          Utp[q] = q == 0 ? U0[0] : l_at(q - 1, ty, tx);
+          sE[(q * TY + ty) * (TX + 2) + tx + 1] = FP[q];
+          sE[((q + 5) * TY + ty) * (TX + 2) + tx + 1] = FM[q];
+          a[q] = FP[q] - FM[q];
         }
-        // x: own parts; the neighbours' parts come from lanes -1 / +1 (the first and the last lane
-        // take theirs from the halo columns after the barrier)
+        if (tid < 2 * TY) {                         // halo columns x = -1 (FP only) and x = TX (FM only)
+          int hy = tid >> 1, side = tid & 1, hx = side ? TX : -1;
+          T Hc[5], Hm[5], Hp[5], hh[5], HF[5];
 #pragma unroll
-        for (int q = 0; q < 5; ++q) { Ua[q] = u_at(q, ty, tx - 1); Ub[q] = u_at(q, ty, tx + 1); }
-        flux_parts<T, 3>(P, 0, U0, Ua, Ub, hf, l_at(4, ty, tx), FP, FM);
+          for (int q = 0; q < 5; ++q) { Hc[q] = u_at(q, hy, hx); Hm[q] = u_at(q, hy, hx - 1); Hp[q] = u_at(q, hy, hx + 1); }
+          hh[0] = Hc[0];
+#pragma unroll
+          for (int q = 1; q < 5; ++q) hh[q] = (T)0.5 * (Hc[q] + l_at(q - 1, hy, hx));
+          T hxi = l_at(4, hy, hx);
+          if (side) {
+            flux_parts<T, 2>(P, 0, Hc, Hm, Hp, hh, hxi, HF, HF);
+#pragma unroll
+            for (int q = 0; q < 5; ++q) sE[((q + 5) * TY + hy) * (TX + 2) + TX + 1] = HF[q];
+          } else {
+            flux_parts<T, 1>(P, 0, Hc, Hm, Hp, hh, hxi, HF, HF);
+#pragma unroll
+            for (int q = 0; q < 5; ++q) sE[(q * TY + hy) * (TX + 2) + 0] = HF[q];
+          }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < 5; ++q)
+          a[q] += sE[((q + 5) * TY + ty) * (TX + 2) + tx + 2] - sE[(q * TY + ty) * (TX + 2) + tx];
+        __syncthreads();
+      }
+      // ---- y axis -------------------------------------------------------------
+      {
+        T Uy0[5], Uy1[5], FP[5], FM[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { Uy0[q] = u_at(q, ty - 1, tx); Uy1[q] = u_at(q, ty + 1, tx); }
+        flux_parts<T, 3>(P, 1, U0, Uy0, Uy1, hf, l_at(5, ty, tx), FP, FM);
+        // exchange layout: [q][ty+1][tx], rows -1..TY, row pitch TX
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
-          T fpl = __shfl_up_sync(0xffffffffu, FP[q], 1);
-          T fmr = __shfl_down_sync(0xffffffffu, FM[q], 1);
-          if (tx == 0) fpl = (T)0;
-          if (tx == TX - 1) fmr = (T)0;
-          acc[q] += (FP[q] - FM[q]) + (fmr - fpl);
+          sE[(q * (TY + 2) + ty + 1) * TX + tx] = FP[q];
+          sE[((q + 5) * (TY + 2) + ty + 1) * TX + tx] = FM[q];
+          a[q] += FP[q] - FM[q];
         }
-        // y: own parts; FP of row r goes to [q][r+1], FM of row r to [5+q][r]
+        if (tid >= TX * TY - 2 * TX) {               // halo rows y = -1 (FP only) and y = TY (FM only): last two warps
+          int t = tid - (TX * TY - 2 * TX);
+          int hx = t % TX, side = t / TX, hy = side ? TY : -1;
+          T Hc[5], Hm[5], Hp[5], hh[5], HF[5];
 #pragma unroll
-        for (int q = 0; q < 5; ++q) { Ua[q] = u_at(q, ty - 1, tx); Ub[q] = u_at(q, ty + 1, tx); }
-        flux_parts<T, 3>(P, 1, U0, Ua, Ub, hf, l_at(5, ty, tx), FP, FM);
+          for (int q = 0; q < 5; ++q) { Hc[q] = u_at(q, hy, hx); Hm[q] = u_at(q, hy - 1, hx); Hp[q] = u_at(q, hy + 1, hx); }
+          hh[0] = Hc[0];
 #pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          sEY[(q * (TY + 1) + ty + 1) * TX + tx] = FP[q];
-          sEY[((q + 5) * (TY + 1) + ty) * TX + tx] = FM[q];
-          acc[q] += FP[q] - FM[q];
+          for (int q = 1; q < 5; ++q) hh[q] = (T)0.5 * (Hc[q] + l_at(q - 1, hy, hx));
+          T hxi = l_at(5, hy, hx);
+          if (side) {
+            flux_parts<T, 2>(P, 1, Hc, Hm, Hp, hh, hxi, HF, HF);
+#pragma unroll
+            for (int q = 0; q < 5; ++q) sE[((q + 5) * (TY + 2) + TY + 1) * TX + hx] = HF[q];
+          } else {
+            flux_parts<T, 1>(P, 1, Hc, Hm, Hp, hh, hxi, HF, HF);
+#pragma unroll
+            for (int q = 0; q < 5; ++q) sE[(q * (TY + 2) + 0) * TX + hx] = HF[q];
+          }
         }
-      }
+        __syncthreads();
 #pragma unroll
-      for (int q = 0; q < 5; ++q) { FPzp[q] = FPz[q]; Um[q] = U0[q]; }
-    } else if (active) {
-      // halo rows: y part towards the tile, then the x part of one halo column towards the tile
-      const bool lo = ty < 0;
-      T Uc[5], Ua[5], Ub[5], hf[5], HF[5];
-      gather(1, ty, tx, Uc, Ua, Ub, hf);
-      if (lo) {
-        flux_parts<T, 1>(P, 1, Uc, Ua, Ub, hf, l_at(5, ty, tx), HF, HF);
-#pragma unroll
-        for (int q = 0; q < 5; ++q) sEY[(q * (TY + 1) + 0) * TX + tx] = HF[q];
-      } else {
-        flux_parts<T, 2>(P, 1, Uc, Ua, Ub, hf, l_at(5, ty, tx), HF, HF);
-#pragma unroll
-        for (int q = 0; q < 5; ++q) sEY[((q + 5) * (TY + 1) + TY) * TX + tx] = HF[q];
-      }
-      if (tx < TY) {
-        const int hx = lo ? -1 : TX;
-        gather(0, tx, hx, Uc, Ua, Ub, hf);
-        if (lo) {
-          flux_parts<T, 1>(P, 0, Uc, Ua, Ub, hf, l_at(4, tx, hx), HF, HF);
-#pragma unroll
-          for (int q = 0; q < 5; ++q) sEX[q * TY + tx] = HF[q];
-        } else {
-          flux_parts<T, 2>(P, 0, Uc, Ua, Ub, hf, l_at(4, tx, hx), HF, HF);
-#pragma unroll
-          for (int q = 0; q < 5; ++q) sEX[(q + 5) * TY + tx] = HF[q];
-        }
+        for (int q = 0; q < 5; ++q)
+          a[q] += sE[((q + 5) * (TY + 2) + ty + 2) * TX + tx] - sE[(q * (TY + 2) + ty) * TX + tx];
       }
     }
-    __syncthreads();                                   // the parts of plane p are visible
-
-    if (main_row && active) {
+    // z axis: both parts of plane p; U^n of plane p+1 from the other stage
+    T Up[5], FPz[5], FMz[5];
+    mbar_wait(&bar[s ^ 1], (phase >> (s ^ 1)) & 1u);
+    phase ^= 1u << (s ^ 1);
+    {
+      const T* sU1 = (const T*)(sm + S::OFF_U + (s ^ 1) * S::U_STAGE);
+#pragma unroll
+      for (int q = 0; q < 5; ++q) Up[q] = sU1[(q * S::UY + (ty + 2)) * S::BX + (tx + S::HX)];
+    }
+    flux_parts<T, 3>(P, 2, U0, Um, Up, hf, l_at(6, ty, tx), FPz, FMz);
+    // finish cell p-1 (SUE, Eq. (4))
+    if (p - 1 >= z0) {
+      T un[5];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) un[q] = Utp[q] - lam * (acc[q] + FMz[q]);
+      if (inside) {
+        long long c = L.idx(i, j, p - 1);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) UN[c + q * fs] = un[q];
+        T sp = cell_speed_exact<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
+        smax = sp > smax ? sp : smax;
+      }
+    }
+    if (active) {
+      // z: own parts of plane p, FP of plane p-1; FM of plane p+1 is added when it is known
 #pragma unroll
       for (int q = 0; q < 5; ++q) {
-        T fpd = sEY[(q * (TY + 1) + ty) * TX + tx];                  // FP of row ty-1
-        T fmu = sEY[((q + 5) * (TY + 1) + ty + 1) * TX + tx];        // FM of row ty+1
-        T e = fmu - fpd;
-        if (tx == 0) e -= sEX[q * TY + ty];                          // FP of column -1
-        if (tx == TX - 1) e += sEX[(q + 5) * TY + ty];               // FM of column TX
-        acc[q] += e;
+        acc[q] = a[q] + ((FPz[q] - FMz[q]) - FPzp[q]);
+        Utp[q] = q == 0 ? U0[0] : l_at(q - 1, ty, tx);
       }
     }
-    __syncthreads();                                   // everyone is done with stage K and with the exchange buffers
-    if (tid == 0 && p + 2 <= z1) issue(p + 2, K);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { FPzp[q] = FPz[q]; Um[q] = U0[q]; }
+    __syncthreads();                                   // everyone is done with stage s and with sE
+    if (tid == 0 && p + 2 <= z1 + 1) issue(p + 2, s);
   }
   block_max_to_global<T>(smax, smax_out);
 }
