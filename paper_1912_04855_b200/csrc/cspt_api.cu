@@ -235,8 +235,6 @@ bool corr_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
 template <class T>
 bool corr_dispatch(cspt_ctx* c, const Params<T>* P, const T* U) {
   switch (c->corr_variant) {
-    case 1: return corr_variant<T, 32, 16, 2, 4, 1>(c, P, U);
-    case 2: return corr_variant<T, 32, 8, 2, 4, 1>(c, P, U);
     case 3: return corr_variant<T, 32, 8, 2, 4, 3>(c, P, U);
     default: return corr_variant<T, 32, 8, 2, 4, 2>(c, P, U);     // fastest on B200 in both precisions
   }
