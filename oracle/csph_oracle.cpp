@@ -320,6 +320,15 @@ struct Oracle {
     if (a < (T)0 && b < (T)0) return a > b ? a : b;
     return (T)0;
   }
+  // van Leer's harmonic-mean limiter: 2ab/(a+b) where a and b have the same sign, else 0.
+  static T vanleer(T a, T b) {
+    if (a * b > (T)0) return ((T)2 * a * b) / (a + b);
+    return (T)0;
+  }
+  // TVD slope Theta (PAPER.md:78 "should satisfy the TVD-condition"; :133 "different TVD-limiters"):
+  // limiter 0 = minmod (reading G12, the default), 1 = van Leer.
+  int limiter = 0;
+  T slope(T a, T b) const { return limiter == 1 ? vanleer(a, b) : minmod(a, b); }
 
   // ---- O7: FGC, Eq. (8) + pressureless HLL flux (G10-G13) ----
   void fluxes() {
@@ -334,9 +343,9 @@ struct Oracle {
             size_t cL = idx(i, j, k), cR = cL + sd;
             T UL[5], UR[5];
             for (int q = 0; q < 5; ++q) {
-              // TVD slope from U^n (G12: minmod on conserved variables)
-              T thL = minmod((U[q][cL] - U[q][cL - sd]) / h, (U[q][cL + sd] - U[q][cL]) / h);
-              T thR = minmod((U[q][cR] - U[q][cR - sd]) / h, (U[q][cR + sd] - U[q][cR]) / h);
+              // TVD slope from U^n (G12: limiter on conserved variables)
+              T thL = slope((U[q][cL] - U[q][cL - sd]) / h, (U[q][cL + sd] - U[q][cL]) / h);
+              T thR = slope((U[q][cR] - U[q][cR - sd]) / h, (U[q][cR + sd] - U[q][cR]) / h);
               // U^{n+1/2} = (U^n + U~)/2 (G10)
               T hL = (T)0.5 * (U[q][cL] + Ut[q][cL]);
               T hR = (T)0.5 * (U[q][cR] + Ut[q][cR]);
@@ -449,6 +458,13 @@ double orc_compute_dt(void* vh, double cfl) {
 void orc_step(void* vh, double dt) {
   Handle* hd = (Handle*)vh;
   DISPATCH(hd, o->step((T)dt), o->step((T)dt));
+}
+
+// limiter: 0 = minmod (default), 1 = van Leer; other values are ignored
+void orc_set_limiter(void* vh, int limiter) {
+  Handle* hd = (Handle*)vh;
+  if (limiter != 0 && limiter != 1) return;
+  DISPATCH(hd, o->limiter = limiter, o->limiter = limiter);
 }
 
 void orc_get_conserved(void* vh, void* rho, void* mx, void* my, void* mz, void* E) {

@@ -20,6 +20,7 @@ _LIB_PATH = os.path.join(_HERE, "libcsph_oracle.so")
 
 F64, F32 = 0, 1
 BC_PERIODIC, BC_OUTFLOW, BC_INFLOW = 0, 1, 2
+LIMITER_MINMOD, LIMITER_VANLEER = 0, 1
 
 _lib = None
 
@@ -52,6 +53,8 @@ def _load():
     lib.orc_compute_dt.argtypes = [vp, cd]
     lib.orc_compute_dt.restype = cd
     lib.orc_step.argtypes = [vp, cd]
+    lib.orc_set_limiter.argtypes = [vp, ci]
+    lib.orc_set_limiter.restype = None
     lib.orc_step.restype = None
     lib.orc_get_conserved.argtypes = [vp] * 6
     lib.orc_get_conserved.restype = None
@@ -116,6 +119,10 @@ class Oracle:
 
     def compute_dt(self, cfl):
         return float(_load().orc_compute_dt(self._h, float(cfl)))
+
+    def set_limiter(self, limiter):
+        """0 = minmod (default, reading G12), 1 = van Leer."""
+        _load().orc_set_limiter(self._h, int(limiter))
 
     def step(self, dt):
         _load().orc_step(self._h, float(dt))
