@@ -59,6 +59,8 @@ def parse():
     ap.add_argument("--workload", default="turbulence")
     ap.add_argument("--n", type=int, default=None, help="grid size override (default: the config's)")
     ap.add_argument("--dtype", default=None, choices=["f64", "f32"])
+    ap.add_argument("--limiter", default="minmod", choices=["minmod", "vanleer"],
+                    help="TVD slope limiter of the Euler stage (default: the reading the metric is quoted on)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -288,6 +290,7 @@ def run_cspt(args):
     fields = host_fields(w, pin=True)
     s = cspt.Solver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, dtype)
     s.set_state_host(*fields)
+    s.set_limiter(cspt.LIMITER_VANLEER if args.limiter == "vanleer" else cspt.LIMITER_MINMOD)
 
     def barrier():
         torch.cuda.synchronize()
@@ -389,7 +392,7 @@ def run_cspt(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": w.dtype, "data": "synthetic",
-        "config": config_of(w, world),
+        "config": dict(config_of(w, world), limiter=args.limiter),
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "kernels": kern,
         "roofline": roofline, "step_hbm": step_hbm,
     }

@@ -36,6 +36,8 @@ typedef struct cspt_ctx cspt_ctx; /* opaque */
 enum { CSPT_F64 = 0, CSPT_F32 = 1 };
 /* boundary kind per face, order xlo,xhi,ylo,yhi,zlo,zhi (reading G16) */
 enum { CSPT_BC_PERIODIC = 0, CSPT_BC_OUTFLOW = 1, CSPT_BC_INFLOW = 2 };
+/* TVD slope limiter of Eq. (8): minmod is the default (reading G12) */
+enum { CSPT_LIMITER_MINMOD = 0, CSPT_LIMITER_VANLEER = 1 };
 enum { CSPT_OK = 0, CSPT_EINVAL = -1, CSPT_ENOMEM = -2, CSPT_ECUDA = -3, CSPT_ESTATE = -4 };
 
 /* Bytes of device workspace cspt_create needs for this grid (0 if the arguments
@@ -68,6 +70,12 @@ int cspt_set_state_host(cspt_ctx*, const void* rho, const void* u, const void* v
  * Bit-exact and order independent (warp-shuffle + block max + integer atomic max
  * of the IEEE bit pattern).  Writes *dt_host_out; syncs.  EINVAL: cfl <= 0. */
 int cspt_compute_dt(cspt_ctx*, double cfl, double* dt_host_out);
+
+/* Chooses the slope limiter Theta of the piecewise-linear reconstruction, Eq. (8) ("the slope
+ * ... should satisfy the TVD-condition"; "different TVD-limiters"): CSPT_LIMITER_MINMOD (default)
+ * or CSPT_LIMITER_VANLEER (2ab/(a+b) where the one-sided differences a, b agree in sign, else 0).  Takes effect
+ * from the next step.  Host-side only, no device work.  EINVAL: null ctx or unknown limiter. */
+int cspt_set_limiter(cspt_ctx*, int limiter);
 
 /* One full step U^n -> U^{n+1} with time step dt (Eq. (4)-(8)): ghost fill,
  * HFC/SUL predictor, HFC/SUL corrector, FGC, SUE.

@@ -251,8 +251,10 @@ bool make_maps(cspt_ctx* c) {
                               S::BX, S::UY, 5);
   ok = ok && make_field_map(&c->mapL, field<T>(c, S_UT), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 7, S::BX, S::LY, 7);
   if (ok) {
-    ok = cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
-         cudaSuccess;
+    ok = cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
+             cudaSuccess &&
+         cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
+             cudaSuccess;
   }
   ok = ok && corr_dispatch<T>(c, nullptr, nullptr);
   return ok;
@@ -289,8 +291,8 @@ void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
   dim3 grid(gx, gy, (L.nz + zc - 1) / zc);
   DevScalars<T>* sc = scalars<T>(c);
   int ps_ = prof_open(c, K_EULER);
-  k_euler_stream<T, ETX, ETY><<<grid, ETX * ETY, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN,
-                                                                        &sc->smax_bits, zc);
+  auto kern = c->limiter == CSPT_LIMITER_VANLEER ? k_euler_stream<T, ETX, ETY, 1> : k_euler_stream<T, ETX, ETY, 0>;
+  kern<<<grid, ETX * ETY, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN, &sc->smax_bits, zc);
   prof_close(c, ps_);
   c->launches++;
 }
@@ -303,15 +305,10 @@ void run_step(cspt_ctx* c) {
   T* UN = field<T>(c, c->cur ? S_U0 : S_U1);
   DevScalars<T>* sc = scalars<T>(c);
   fill_ghosts<T>(c, U, 5, 0);                                                      // O0
-  long long n0 = (long long)L.nx * L.ny * L.nz;
   launch_predictor<T>(c, P, U);                                                    // O1, O3, O4
   launch_corrector<T>(c, P, U);                                                    // O5, O6
   LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, sc);
-  if (c->legacy_euler)
-    LAUNCH(c, K_EULER, k_euler<T>, blocks_for(n0, TPB), TPB, P, sc, U, field<T>(c, S_UT), field<T>(c, S_XI), UN,
-           &sc->smax_bits);
-  else
-    launch_euler<T>(c, P, U, UN);                                                  // O7, O8 (+O9 epilogue)
+  launch_euler<T>(c, P, U, UN);                                                  // O7, O8 (+O9 epilogue)
   c->cur ^= 1;
   c->smax_valid = true;
 }
@@ -388,7 +385,6 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->corr_variant = getenv("CSPT_CORR_VARIANT") ? atoi(getenv("CSPT_CORR_VARIANT")) : 0;   // tuning switch
   c->have_maps = dtype == CSPT_F64 ? make_maps<double>(c) : make_maps<float>(c);
   if (!c->have_maps) { (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }
-  c->legacy_euler = getenv("CSPT_LEGACY_EULER") != nullptr;
 
   *out = c;
   return CSPT_OK;
@@ -475,6 +471,12 @@ int cspt_compute_dt(cspt_ctx* c, double cfl, double* dt_host_out) {
   if (!c->has_state) return CSPT_ESTATE;
   if (c->cuda_error) return CSPT_ECUDA;
   return DISPATCH(c, compute_dt_t)(c, cfl, dt_host_out);
+}
+
+int cspt_set_limiter(cspt_ctx* c, int limiter) {
+  if (!c || (limiter != CSPT_LIMITER_MINMOD && limiter != CSPT_LIMITER_VANLEER)) return CSPT_EINVAL;
+  c->limiter = limiter;
+  return CSPT_OK;
 }
 
 int cspt_step(cspt_ctx* c, double dt) {

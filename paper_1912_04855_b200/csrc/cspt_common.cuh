@@ -112,7 +112,7 @@ struct cspt_ctx {
   CUtensorMap mapU[2], mapL, mapS;
   bool have_maps;
   int corr_variant;         // tuning switch (env CSPT_CORR_VARIANT): corrector tile variant
-  bool legacy_euler;        // debug switch (env CSPT_LEGACY_EULER): first, unfused Euler kernel
+  int limiter;              // CSPT_LIMITER_*: TVD slope of Eq. (8) in the Euler stage
   // per-kernel device timing (cspt_profile_*): event pairs recorded around each launch
   bool prof_on;
   int prof_used;                    // pairs recorded since the last reset

@@ -26,7 +26,21 @@ __device__ __forceinline__ T minmod_fast(T a, T b) {
 
 // One-sided flux parts of one cell along axis d.  Uc/Um/Up: U^n of the cell and of its -/+
 // neighbours; hf = U^{n+1/2} = (U^n + U~)/2 (G10); xi = xi_d of the cell.
-template <class T, int WANT>   // WANT bit 0: FP, bit 1: FM
+// van Leer's harmonic limiter 2ab/(a+b) for ab > 0, else 0 ("different TVD-limiters").
+template <class T>
+__device__ __forceinline__ T vanleer_fast(T a, T b) {
+  T ab = a * b, sum = a + b;
+  bool ok = ab > (T)0 && fabs(sum) > Fast<T>::tiny() * (T)1e20;      // keeps the reciprocal seed normal
+  T r = ((T)2 * ab) * Fast<T>::rcp(ok ? sum : (T)1);
+  return ok ? r : (T)0;
+}
+// TVD slope of Eq. (8): LIM 0 = minmod (reading G12), 1 = van Leer
+template <class T, int LIM>
+__device__ __forceinline__ T tvd_slope(T a, T b) {
+  return LIM == 1 ? vanleer_fast<T>(a, b) : minmod_fast<T>(a, b);
+}
+
+template <class T, int WANT, int LIM>   // WANT bit 0: FP, bit 1: FM
 __device__ __forceinline__ void flux_parts(const Params<T>& P, int d, const T* Uc, const T* Um, const T* Up, const T* hf,
                                            T xi, T* FP, T* FM) {
   T cP = ((T)0.5 * (P.h - xi)) * P.inv_h;      // (h - xi)/2 * (1/h): slope is minmod(dU)/h (Eq. (8))
@@ -34,7 +48,7 @@ __device__ __forceinline__ void flux_parts(const Params<T>& P, int d, const T* U
   T UL[5], UR[5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) {
-    T mm = minmod_fast<T>(Uc[q] - Um[q], Up[q] - Uc[q]);      // G12
+    T mm = tvd_slope<T, LIM>(Uc[q] - Um[q], Up[q] - Uc[q]);      // G12
     if (WANT & 1) UL[q] = hf[q] + cP * mm;
     if (WANT & 2) UR[q] = hf[q] - cM * mm;
   }
@@ -71,7 +85,7 @@ struct EulerSmem {
   static constexpr int BYTES = OFF_BAR + 64 + 128;  // + slack for the 128-byte alignment of the base
 };
 
-template <class T, int TX, int TY>
+template <class T, int TX, int TY, int LIM>
 __global__ void __launch_bounds__(TX* TY, 2)
 k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL, Params<T> P,
                const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, T* __restrict__ UN,
@@ -147,7 +161,7 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
         T Ux0[5], Ux1[5], FP[5], FM[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) { Ux0[q] = u_at(q, ty, tx - 1); Ux1[q] = u_at(q, ty, tx + 1); }
-        flux_parts<T, 3>(P, 0, U0, Ux0, Ux1, hf, l_at(4, ty, tx), FP, FM);
+        flux_parts<T, 3, LIM>(P, 0, U0, Ux0, Ux1, hf, l_at(4, ty, tx), FP, FM);
         // exchange layout: [q][ty][tx+1], FP in 0..4, FM in 5..9, row pitch TX+2
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
@@ -165,11 +179,11 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
           for (int q = 1; q < 5; ++q) hh[q] = (T)0.5 * (Hc[q] + l_at(q - 1, hy, hx));
           T hxi = l_at(4, hy, hx);
           if (side) {
-            flux_parts<T, 2>(P, 0, Hc, Hm, Hp, hh, hxi, HF, HF);
+            flux_parts<T, 2, LIM>(P, 0, Hc, Hm, Hp, hh, hxi, HF, HF);
 #pragma unroll
             for (int q = 0; q < 5; ++q) sE[((q + 5) * TY + hy) * (TX + 2) + TX + 1] = HF[q];
           } else {
-            flux_parts<T, 1>(P, 0, Hc, Hm, Hp, hh, hxi, HF, HF);
+            flux_parts<T, 1, LIM>(P, 0, Hc, Hm, Hp, hh, hxi, HF, HF);
 #pragma unroll
             for (int q = 0; q < 5; ++q) sE[(q * TY + hy) * (TX + 2) + 0] = HF[q];
           }
@@ -185,7 +199,7 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
         T Uy0[5], Uy1[5], FP[5], FM[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) { Uy0[q] = u_at(q, ty - 1, tx); Uy1[q] = u_at(q, ty + 1, tx); }
-        flux_parts<T, 3>(P, 1, U0, Uy0, Uy1, hf, l_at(5, ty, tx), FP, FM);
+        flux_parts<T, 3, LIM>(P, 1, U0, Uy0, Uy1, hf, l_at(5, ty, tx), FP, FM);
         // exchange layout: [q][ty+1][tx], rows -1..TY, row pitch TX
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
@@ -204,11 +218,11 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
           for (int q = 1; q < 5; ++q) hh[q] = (T)0.5 * (Hc[q] + l_at(q - 1, hy, hx));
           T hxi = l_at(5, hy, hx);
           if (side) {
-            flux_parts<T, 2>(P, 1, Hc, Hm, Hp, hh, hxi, HF, HF);
+            flux_parts<T, 2, LIM>(P, 1, Hc, Hm, Hp, hh, hxi, HF, HF);
 #pragma unroll
             for (int q = 0; q < 5; ++q) sE[((q + 5) * (TY + 2) + TY + 1) * TX + hx] = HF[q];
           } else {
-            flux_parts<T, 1>(P, 1, Hc, Hm, Hp, hh, hxi, HF, HF);
+            flux_parts<T, 1, LIM>(P, 1, Hc, Hm, Hp, hh, hxi, HF, HF);
 #pragma unroll
             for (int q = 0; q < 5; ++q) sE[(q * (TY + 2) + 0) * TX + hx] = HF[q];
           }
@@ -228,7 +242,7 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
 #pragma unroll
       for (int q = 0; q < 5; ++q) Up[q] = sU1[(q * S::UY + (ty + 2)) * S::BX + (tx + S::HX)];
     }
-    flux_parts<T, 3>(P, 2, U0, Um, Up, hf, l_at(6, ty, tx), FPz, FMz);
+    flux_parts<T, 3, LIM>(P, 2, U0, Um, Up, hf, l_at(6, ty, tx), FPz, FMz);
     // finish cell p-1 (SUE, Eq. (4))
     if (p - 1 >= z0) {
       T un[5];

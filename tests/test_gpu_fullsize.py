@@ -73,12 +73,13 @@ def window_box(w, lo, size, pad):
     return box
 
 
-def check_windows(cspt, oracle_mod, w, windows, steps, tol, size=(48, 48, 48)):
+def check_windows(cspt, oracle_mod, w, windows, steps, tol, size=(48, 48, 48), limiter=0):
     import torch
     dev = torch.device("cuda", torch.cuda.current_device())
     s = cspt.Solver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, cspt.F64 if w.dtype == "f64" else cspt.F32)
     f = device_fields(w, dev)
     s.set_state(*f)
+    s.set_limiter(limiter)
     del f
     torch.cuda.empty_cache()
     dts = [s.step_cfl(w.cfl, want_dt=True) for _ in range(steps)]
@@ -100,6 +101,7 @@ def check_windows(cspt, oracle_mod, w, windows, steps, tol, size=(48, 48, 48)):
                          w.dtype, None)
         o = make_oracle(oracle_mod, ww, dtype="f64")
         o.set_state(*[np.asarray(a, dtype=np.float64) for a in fw])
+        o.set_limiter(limiter)
         for dt in dts:
             o.step(dt)
         ref = o.get_conserved()
@@ -137,6 +139,11 @@ def test_cfg3_well_256_windows(cspt, oracle_mod):
 def test_cfg4_turbulence_512_windows(cspt, oracle_mod, dtype):
     w = wl.turbulence(dtype=dtype)
     check_windows(cspt, oracle_mod, w, corner_and_centre_windows(w), 6, TOL64 if dtype == "f64" else TOL32)
+
+
+def test_cfg4_turbulence_512_vanleer_windows(cspt, oracle_mod):
+    w = wl.turbulence()
+    check_windows(cspt, oracle_mod, w, corner_and_centre_windows(w)[:2], 6, TOL64, limiter=cspt.LIMITER_VANLEER)
 
 
 def test_cfg5_disk_1024_windows(cspt, oracle_mod):

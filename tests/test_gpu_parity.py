@@ -48,7 +48,7 @@ def field_errors(gpu, orc):
     return errs
 
 
-def run_pair(cspt, orc_mod, w, steps, tol, gpu_dtype=None, fields=None, check_dt=True):
+def run_pair(cspt, orc_mod, w, steps, tol, gpu_dtype=None, fields=None, check_dt=True, limiter=0):
     """Steps both sides with the oracle's dt sequence; returns (solver, oracle)."""
     f = fields if fields is not None else w.fields()
     gd = gpu_dtype or w.dtype
@@ -56,6 +56,9 @@ def run_pair(cspt, orc_mod, w, steps, tol, gpu_dtype=None, fields=None, check_dt
     o.set_state(*[np.asarray(a, dtype=np.float64) for a in f] if gd == "f32" else f)
     s = make_solver(cspt, w, dtype=gd)
     s.set_state(*f)
+    if limiter:
+        o.set_limiter(limiter)
+        s.set_limiter(limiter)
     if check_dt and gd == "f64":
         assert s.compute_dt(w.cfl) == o.compute_dt(w.cfl)          # bit-exact on the same input
     for n in range(steps):
@@ -160,6 +163,38 @@ def test_cfg5_disk_vacuum(cspt, oracle_mod, dtype):
             assert np.array_equal(a.cpu().numpy(), b)            # primitives use exactly rounded operations
     m = s.get_vacuum_mask().cpu().numpy()
     assert 0 < m.sum() < m.size                                  # the case really has gas and vacuum
+
+
+# ---- the limiter switch: van Leer on both sides --------------------------------------
+@pytest.mark.parametrize("dims,bc,dtype", [
+    ((40, 37, 21), [0] * 6, "f64"),
+    ((33, 18, 45), [1, 2, 0, 0, 1, 1], "f64"),
+    ((40, 37, 21), [0] * 6, "f32"),
+])
+def test_vanleer_random_smooth(cspt, oracle_mod, dims, bc, dtype):
+    w = wl.random_smooth(*dims, bc=bc, dtype=dtype)
+    run_pair(cspt, oracle_mod, w, 10, TOL64 if dtype == "f64" else TOL32, limiter=cspt.LIMITER_VANLEER)
+
+
+def test_vanleer_sod_and_disk(cspt, oracle_mod):
+    run_pair(cspt, oracle_mod, wl.sod(axis=1), 10, TOL64, limiter=cspt.LIMITER_VANLEER)
+    run_pair(cspt, oracle_mod, wl.disk(n=40, dtype="f64"), 10, TOL64, limiter=cspt.LIMITER_VANLEER)
+
+
+def test_limiter_switch_changes_the_result_and_rejects_unknown_values(cspt, oracle_mod):
+    import torch
+    w = wl.random_smooth(20, 12, 9)
+    a, b = make_solver(cspt, w), make_solver(cspt, w)
+    a.set_state(*w.fields())
+    b.set_state(*w.fields())
+    b.set_limiter(cspt.LIMITER_VANLEER)
+    a.step(1e-3)
+    b.step(1e-3)
+    assert not torch.equal(a.get_conserved()[0], b.get_conserved()[0])
+    b.set_limiter(cspt.LIMITER_MINMOD)
+    with pytest.raises(cspt.CsptError) as e:
+        b.set_limiter(7)
+    assert e.value.code == cspt.EINVAL
 
 
 # ---- degenerate cases ---------------------------------------------------------------------------
