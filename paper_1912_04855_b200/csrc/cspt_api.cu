@@ -200,10 +200,13 @@ constexpr int ETX = 32;
 template <class T> struct EulerTile { static constexpr int TY = 8; };
 
 int pick_zchunk(int tiles, int nz) {
-  // enough CTAs for ~8 waves of 2 CTAs per SM, but at least 16 planes per CTA (2 extra planes per chunk)
+  // enough CTAs for ~8 waves of 2 CTAs per SM, at least 16 planes per CTA (2 extra planes per chunk) and at
+  // most 64: CTAs of neighbouring tiles then stay close in z, so the halo rows they share are still in L2
+  // (1024^3 fp32: corrector 41.5 -> 32.1 ms against one chunk per column)
   int want = (148 * 2 * 8 + tiles - 1) / tiles;
   int zc = (nz + want - 1) / want;
   if (zc < 16) zc = 16;
+  if (zc > 64) zc = 64;
   if (zc > nz) zc = nz;
   return zc;
 }
