@@ -87,17 +87,30 @@ struct Oracle {
       for (int c = 0; c < 5; ++c) A(F[d][c]);
     }
     for (int c = 0; c < 4; ++c) A(Q[c]);
-    // g^(q) = -W'(q)/q of the Monaghan cubic spline with smoothing length h:
-    //   3 - 2.25 q          (q < 1)
-    //   0.75 (2-q)^2 / q    (1 <= q < 2)
-    //   0                   (q >= 2)
-    // S0' = sum over the 26 lattice neighbours of g^(|o|) o_x^2, so that the
-    // undisplaced operator reproduces linear fields exactly (reading G5).
-    double s2 = std::sqrt(2.0), s3 = std::sqrt(3.0);
-    double g1 = 0.75, g2 = 0.75 * (2.0 - s2) * (2.0 - s2) / s2, g3 = 0.75 * (2.0 - s3) * (2.0 - s3) / s3;
+    set_kernel(0);
+  }
+
+  // Smoothing kernel W (PAPER.md:68 leaves it open; :133 "different smoothing kernels can be used"):
+  //   kernel 0 (reading G5, the default): Monaghan cubic spline with smoothing length h,
+  //       g^(q) = -W'(q)/q = 3 - 2.25 q (q < 1),  0.75 (2-q)^2 / q (1 <= q < 2),  0 (q >= 2)
+  //   kernel 1: W ~ (1 - q^2/4)^5 on q < 2, for which -W'(q)/q ~ (1 - q^2/4)^4
+  //       needs no square root (any constant factor cancels against S0')
+  // S0' = sum over the 26 lattice neighbours of g^(|o|) o_x^2, so that the undisplaced operator
+  // reproduces linear fields exactly (reading G5).
+  int kernel = 0;
+  static double ghat_d(int kernel, double q) {
+    if (kernel == 1) { double t = 1.0 - 0.25 * q * q; return q < 2.0 ? (t * t) * (t * t) : 0.0; }
+    if (q < 1.0) return 3.0 - 2.25 * q;
+    if (q < 2.0) return 0.75 * (2.0 - q) * (2.0 - q) / q;
+    return 0.0;
+  }
+  void set_kernel(int k) {
+    kernel = k;
+    double g1 = ghat_d(k, 1.0), g2 = ghat_d(k, std::sqrt(2.0)), g3 = ghat_d(k, std::sqrt(3.0));
     double S = 2.0 * g1 + 8.0 * g2 + 8.0 * g3;
     S0p = (T)S;
     a_shell[0] = 0; a_shell[1] = (T)(g1 / S); a_shell[2] = (T)(g2 / S); a_shell[3] = (T)(g3 / S);
+    if (has_state) force();          // f = -D[psi] uses the lattice weights
   }
 
   // ---- O0: ghost cells, axis by axis (reading G16) ---------------------------
@@ -217,7 +230,10 @@ struct Oracle {
   // kernel weight w(r) = g^(r/h) / (S0' h^2)   (reading G5)
   T kernel_w(T r) const {
     T q = r / h, g;
-    if (q < (T)1) g = (T)3 - (T)2.25 * q;
+    if (kernel == 1) {
+      T t = (T)1 - (T)0.25 * q * q;
+      g = q < (T)2 ? (t * t) * (t * t) : (T)0;
+    } else if (q < (T)1) g = (T)3 - (T)2.25 * q;
     else if (q < (T)2) g = (T)0.75 * ((T)2 - q) * ((T)2 - q) / q;
     else g = (T)0;
     return g / (S0p * h * h);
@@ -458,6 +474,13 @@ double orc_compute_dt(void* vh, double cfl) {
 void orc_step(void* vh, double dt) {
   Handle* hd = (Handle*)vh;
   DISPATCH(hd, o->step((T)dt), o->step((T)dt));
+}
+
+// smoothing kernel: 0 = cubic spline (default), 1 = (1 - q^2/4)^5; other values are ignored
+void orc_set_kernel(void* vh, int kernel) {
+  Handle* hd = (Handle*)vh;
+  if (kernel != 0 && kernel != 1) return;
+  DISPATCH(hd, o->set_kernel(kernel), o->set_kernel(kernel));
 }
 
 // limiter: 0 = minmod (default), 1 = van Leer; other values are ignored

@@ -21,6 +21,7 @@ _LIB_PATH = os.path.join(_HERE, "libcsph_oracle.so")
 F64, F32 = 0, 1
 BC_PERIODIC, BC_OUTFLOW, BC_INFLOW = 0, 1, 2
 LIMITER_MINMOD, LIMITER_VANLEER = 0, 1
+KERNEL_CUBIC_SPLINE, KERNEL_POLY5 = 0, 1
 
 _lib = None
 
@@ -54,6 +55,8 @@ def _load():
     lib.orc_compute_dt.restype = cd
     lib.orc_step.argtypes = [vp, cd]
     lib.orc_set_limiter.argtypes = [vp, ci]
+    lib.orc_set_kernel.argtypes = [vp, ci]
+    lib.orc_set_kernel.restype = None
     lib.orc_set_limiter.restype = None
     lib.orc_step.restype = None
     lib.orc_get_conserved.argtypes = [vp] * 6
@@ -119,6 +122,10 @@ class Oracle:
 
     def compute_dt(self, cfl):
         return float(_load().orc_compute_dt(self._h, float(cfl)))
+
+    def set_kernel(self, kernel):
+        """0 = cubic spline (default, reading G5), 1 = W ~ (1 - q^2/4)^5 (no square root)."""
+        _load().orc_set_kernel(self._h, int(kernel))
 
     def set_limiter(self, limiter):
         """0 = minmod (default, reading G12), 1 = van Leer."""

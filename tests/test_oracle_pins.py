@@ -44,18 +44,25 @@ def _W_m4(r, h):
     return np.where(q < 1, 1 - 1.5 * q ** 2 + 0.75 * q ** 3, np.where(q < 2, 0.25 * (2 - q) ** 3, 0.0))
 
 
-def _gradW(d, h):
+def _W_poly5(r, h):
+    """W ~ (1 - q^2/4)^5 on q < 2 (the square-root-free alternative)."""
+    q = r / h
+    return np.where(q < 2, (1 - 0.25 * q ** 2) ** 5, 0.0)
+
+
+def _gradW(d, h, W=_W_m4):
     """grad_i W(|r_i - r_j|) by central differences of the textbook W (d = r_i - r_j)."""
     eps = 1e-6 * h
     g = np.zeros(3)
     for a in range(3):
         e = np.zeros(3)
         e[a] = eps
-        g[a] = (_W_m4(np.linalg.norm(d + e), h) - _W_m4(np.linalg.norm(d - e), h)) / (2 * eps)
+        g[a] = (W(np.linalg.norm(d + e), h) - W(np.linalg.norm(d - e), h)) / (2 * eps)
     return g
 
 
-def test_Q_brute_force_all_pairs(oracle_mod):
+@pytest.mark.parametrize("kernel", [0, 1])
+def test_Q_brute_force_all_pairs(oracle_mod, kernel):
     """PAPER.md:66 Eq. (7) on a 4^3 periodic box: every pair (i,i') with minimum-image
     lattice offset in {-1,0,1}^3, displaced particles, grad W differentiated numerically
     from the textbook spline, normalised so that the undisplaced operator differentiates
@@ -69,6 +76,8 @@ def test_Q_brute_force_all_pairs(oracle_mod):
     psi = 0.3 * rng.random(shape)
     xi = [0.3 * h * (rng.random(shape) - 0.5) for _ in range(3)]
     o = _custom(n, n, n, h, gamma, [0] * 6, (rho, u, v, w, p, psi), oracle_mod)
+    o.set_kernel(kernel)
+    W = _W_m4 if kernel == 0 else _W_poly5
     Q = o.eval_Q(xi)
     fx, fy, fz = o.eval_force()
 
@@ -77,7 +86,7 @@ def test_Q_brute_force_all_pairs(oracle_mod):
     c = 0.0
     for (ox, oy, oz) in offs:
         d = -h * np.array([ox, oy, oz], float)
-        c += (ox * h) * _gradW(d, h)[0]      # SPH gradient of q = x: sum_j q_j grad_i W
+        c += (ox * h) * _gradW(d, h, W)[0]      # SPH gradient of q = x: sum_j q_j grad_i W
     norm = 1.0 / c
 
     phi = np.sqrt(2 * p)
@@ -94,7 +103,7 @@ def test_Q_brute_force_all_pairs(oracle_mod):
                 for (ox, oy, oz) in offs:
                     kk, jj, ii = (k + oz) % n, (j + oy) % n, (i + ox) % n
                     d = -h * np.array([ox, oy, oz], float) + xiv[k, j, i] - xiv[kk, jj, ii]
-                    gw = _gradW(d, h) * norm
+                    gw = _gradW(d, h, W) * norm
                     sm += phi[kk, jj, ii] * gw
                     se += phi[kk, jj, ii] * np.dot(0.5 * (vel[k, j, i] + vel[kk, jj, ii]), gw)
                 Qm[k, j, i] = -phi[k, j, i] * sm + rho[k, j, i] * f[k, j, i]
@@ -297,6 +306,73 @@ def test_advected_sine_convergence(oracle_mod):
     orders = [math.log2(errs[i] / errs[i + 1]) for i in range(2)]
     assert errs[0] < 5e-3 and errs[2] < 4e-4, errs
     assert orders[0] > 1.6 and orders[1] > 1.75, (errs, orders)
+
+
+# ---- the smoothing-kernel switch (PAPER.md:68 leaves W open, :133 "different smoothing kernels can be used";
+# SURVEY 8(f) NEXT-1): W ~ (1 - q^2/4)^5, whose -W'/q needs no square root -----------------------------------
+def test_poly5_kernel_lattice_constants_and_linear_exactness(oracle_mod):
+    n, h = 8, 0.125
+    z, y, x = np.meshgrid(*[(np.arange(n) + 0.5) * h] * 3, indexing="ij")
+    one = np.ones_like(x)
+    lin = 0.7 * x - 1.3 * y + 0.4 * z + 2.0
+    o = _custom(n, n, n, h, 1.4, [1] * 6, (one, 0 * one, 0 * one, 0 * one, one, lin), oracle_mod)
+    o.set_kernel(1)
+    fx, fy, fz = o.eval_force()
+    assert np.max(np.abs(fx + 0.7)) < 1e-13 and np.max(np.abs(fy - 1.3)) < 1e-13 and np.max(np.abs(fz + 0.4)) < 1e-13
+    a_f, a_e, a_c, S0p = o.lattice_constants()
+    g = [(1 - 0.25 * m) ** 4 for m in (1, 2, 3)]                    # closed form at |o|^2 = 1, 2, 3
+    S = 2 * g[0] + 8 * g[1] + 8 * g[2]
+    assert abs(S0p - S) < 1e-15 and abs(S - (2 * 0.31640625 + 8 * 0.0625 + 8 * 0.00390625)) < 1e-15
+    assert max(abs(a_f - g[0] / S), abs(a_e - g[1] / S), abs(a_c - g[2] / S)) < 4e-16
+    assert abs(2 * a_f + 8 * a_e + 8 * a_c - 1.0) < 1e-15
+
+
+def test_poly5_kernel_equilibrium_conservation_stability(oracle_mod):
+    # exact discrete Gamma = 2 equilibrium (G8 holds for any lattice weights)
+    w = wl.well(n=16, variant="gamma2")
+    o = make_oracle(oracle_mod, w)
+    f0 = w.fields()
+    o.set_state(*f0)
+    o.set_kernel(1)
+    run_to(o, w.cfl, steps=30)
+    rho, u, v, ww, p = o.get_state()
+    assert max(np.max(np.abs(a)) for a in (u, v, ww)) < 1e-13
+    assert np.max(np.abs(rho / f0[0] - 1)) < 1e-13
+    # conservation to round-off (pair antisymmetry does not depend on the kernel)
+    w = wl.random_smooth(12, 10, 8, with_psi=False)
+    o = make_oracle(oracle_mod, w)
+    o.set_state(*w.fields())
+    o.set_kernel(1)
+    s0 = [float(np.sum(a)) for a in o.get_conserved()]
+    a0 = [float(np.sum(np.abs(a))) for a in o.get_conserved()]
+    run_to(o, w.cfl, steps=10)
+    for b, a, sc in zip(s0, [float(np.sum(a)) for a in o.get_conserved()], a0):
+        assert abs(a - b) <= 2e-14 * sc, (a, b)
+    # noise at rest stays small (the kernels the survey's probe found unstable grow by orders of magnitude)
+    n = 12
+    rng = np.random.default_rng(3)
+    shape = (n, n, n)
+    rho = 1 + 1e-3 * (rng.random(shape) - 0.5)
+    p = 1 + 1e-3 * (rng.random(shape) - 0.5)
+    z = np.zeros(shape)
+    o = _custom(n, n, n, 1.0 / n, 1.4, [0] * 6, (rho, z, z, z, p, z), oracle_mod)
+    o.set_kernel(1)
+    run_to(o, 0.4, steps=150)
+    _, u, v, ww, _ = o.get_state()
+    assert math.sqrt(float(np.mean(u * u + v * v + ww * ww))) < 3e-4
+
+
+def test_poly5_kernel_sod_vs_exact_riemann(oracle_mod):
+    import exact_riemann as er
+    w = wl.sod()
+    o = make_oracle(oracle_mod, w)
+    o.set_state(*w.fields())
+    o.set_kernel(1)
+    run_to(o, w.cfl, t_end=w.t_end)
+    rho = o.get_state()[0][0, 0, :]
+    x = (np.arange(w.nx) + 0.5) / w.nx
+    re, _, _ = er.sample((x - 0.5) / w.t_end, 1.0, 0.0, 1.0, 0.125, 0.0, 0.1, 1.4)
+    assert float(np.mean(np.abs(rho - re))) < 1.5e-2
 
 
 # ---- the TVD limiter switch (PAPER.md:78 "should satisfy the TVD-condition", :133 "different TVD-limiters";
