@@ -61,6 +61,8 @@ def parse():
     ap.add_argument("--dtype", default=None, choices=["f64", "f32"])
     ap.add_argument("--limiter", default="minmod", choices=["minmod", "vanleer"],
                     help="TVD slope limiter of the Euler stage (default: the reading the metric is quoted on)")
+    ap.add_argument("--kernel", default="cubic", choices=["cubic", "poly5"],
+                    help="smoothing kernel W of Eq. (7) (default: the reading the metric is quoted on)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -289,6 +291,8 @@ def run_cspt(args):
     dtype = cspt.F64 if w.dtype == "f64" else cspt.F32
     fields = host_fields(w, pin=True)
     s = cspt.Solver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, dtype)
+    if args.kernel == "poly5":
+        s.set_kernel(cspt.KERNEL_POLY5)
     s.set_state_host(*fields)
     s.set_limiter(cspt.LIMITER_VANLEER if args.limiter == "vanleer" else cspt.LIMITER_MINMOD)
 
@@ -373,13 +377,14 @@ def run_cspt(args):
         # (FMA = 2) over the launch time, against lanes x 2 flop x SMs x max SM clock
         lanes = 64 if w.dtype == "f64" else 128
         apeak = 148 * lanes * 2 * 1.965e9 / 1e12
-        aach = KERNEL_FLOPS[dom] * w.cells / (dom_ms * 1e-3) / 1e12
+        flops_cell = KERNEL_FLOPS[dom] if args.kernel == "cubic" else 26 * 27 + 60    # poly5: no 1/sqrt, 3-op spline
+        aach = flops_cell * w.cells / (dom_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": dom, "achieved": aach, "peak": apeak, "unit": "TFLOP/s",
                     "frac": aach / apeak, "traffic": traffic,
                     "peak_source": "derived: 148 SMs x %d %s lanes x 2 flop x 1965 MHz (DESIGN.md section 7; "
                                    "measured 63.4 DFMA / 120.9 FFMA per clock per SM, profiles/r1a_launches_baseline.md)"
                                    % (lanes, w.dtype),
-                    "algorithmic_flops_per_cell": KERNEL_FLOPS[dom], "kernel_ms": dom_ms,
+                    "algorithmic_flops_per_cell": flops_cell, "kernel_ms": dom_ms,
                     "share_of_step": (prof[dom][0] / args.steps) / step_ms, "hbm": hbm}
     else:
         roofline = dict(hbm, bound="hbm", kernel=dom, traffic=traffic, kernel_ms=dom_ms,
@@ -392,7 +397,7 @@ def run_cspt(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": w.dtype, "data": "synthetic",
-        "config": dict(config_of(w, world), limiter=args.limiter),
+        "config": dict(config_of(w, world), limiter=args.limiter, kernel=args.kernel),
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "kernels": kern,
         "roofline": roofline, "step_hbm": step_hbm,
     }

@@ -38,6 +38,8 @@ enum { CSPT_F64 = 0, CSPT_F32 = 1 };
 enum { CSPT_BC_PERIODIC = 0, CSPT_BC_OUTFLOW = 1, CSPT_BC_INFLOW = 2 };
 /* TVD slope limiter of Eq. (8): minmod is the default (reading G12) */
 enum { CSPT_LIMITER_MINMOD = 0, CSPT_LIMITER_VANLEER = 1 };
+/* smoothing kernel W of Eq. (7) (PAPER.md:68 leaves it open, :133): the cubic spline is the default (reading G5) */
+enum { CSPT_KERNEL_CUBIC_SPLINE = 0, CSPT_KERNEL_POLY5 = 1 };
 enum { CSPT_OK = 0, CSPT_EINVAL = -1, CSPT_ENOMEM = -2, CSPT_ECUDA = -3, CSPT_ESTATE = -4 };
 
 /* Bytes of device workspace cspt_create needs for this grid (0 if the arguments
@@ -70,6 +72,14 @@ int cspt_set_state_host(cspt_ctx*, const void* rho, const void* u, const void* v
  * Bit-exact and order independent (warp-shuffle + block max + integer atomic max
  * of the IEEE bit pattern).  Writes *dt_host_out; syncs.  EINVAL: cfl <= 0. */
 int cspt_compute_dt(cspt_ctx*, double cfl, double* dt_host_out);
+
+/* Chooses the smoothing kernel W of the SPH sums of Eq. (7) ("different smoothing kernels can be
+ * used"): CSPT_KERNEL_CUBIC_SPLINE (default; Monaghan M4 with smoothing length h) or
+ * CSPT_KERNEL_POLY5, W ~ (1 - q^2/4)^5 on q = r/h < 2, whose -W'(q)/q ~ (1 - q^2/4)^4 needs no square root.
+ * Both are normalised on the lattice so that the undisplaced operator is exact for linear fields (G5).
+ * The external force f = -D[psi] depends on the kernel's lattice weights, so a CHANGE of kernel discards the
+ * state: call it before cspt_set_state.  Host-side only.  EINVAL: null ctx or unknown kernel. */
+int cspt_set_kernel(cspt_ctx*, int kernel);
 
 /* Chooses the slope limiter Theta of the piecewise-linear reconstruction, Eq. (8) ("the slope
  * ... should satisfy the TVD-condition"; "different TVD-limiters"): CSPT_LIMITER_MINMOD (default)

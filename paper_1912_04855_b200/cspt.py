@@ -12,6 +12,7 @@ LIB_PATH = os.path.join(_HERE, "libcspt.so")
 F64, F32 = 0, 1
 BC_PERIODIC, BC_OUTFLOW, BC_INFLOW = 0, 1, 2
 LIMITER_MINMOD, LIMITER_VANLEER = 0, 1
+KERNEL_CUBIC_SPLINE, KERNEL_POLY5 = 0, 1
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 
 # every symbol include/cspt.h declares: (name, restype, argtypes)
@@ -23,6 +24,7 @@ SYMBOLS = [
     ("cspt_set_state", _ci, [_vp] * 7),
     ("cspt_set_state_host", _ci, [_vp] * 7),
     ("cspt_compute_dt", _ci, [_vp, _cd, _pd]),
+    ("cspt_set_kernel", _ci, [_vp, _ci]),
     ("cspt_set_limiter", _ci, [_vp, _ci]),
     ("cspt_step", _ci, [_vp, _cd]),
     ("cspt_step_cfl", _ci, [_vp, _cd, _pd]),
@@ -145,6 +147,9 @@ class Solver:
         out = ctypes.c_double()
         _check(lib().cspt_compute_dt(self._h, float(cfl), ctypes.byref(out)), "cspt_compute_dt")
         return out.value
+
+    def set_kernel(self, kernel):
+        _check(lib().cspt_set_kernel(self._h, int(kernel)), "cspt_set_kernel")
 
     def set_limiter(self, limiter):
         _check(lib().cspt_set_limiter(self._h, int(limiter)), "cspt_set_limiter")

@@ -49,9 +49,11 @@ template <class T> Params<T> make_params(const cspt_ctx* c) {
   P.gamma = (T)c->gamma;
   P.rho_vac = (T)1e-12;
   P.inv_h = (T)1 / P.h;
-  // Monaghan cubic spline, smoothing length h: g^(q) = -W'(q)/q (G5)
+  // g^(q) = -W'(q)/q at the lattice distances 1, sqrt 2, sqrt 3: Monaghan cubic spline with smoothing length h
+  // (G5), or W ~ (1 - q^2/4)^5 for which g^ ~ (1 - q^2/4)^4
   double s2 = sqrt(2.0), s3 = sqrt(3.0);
   double g1 = 0.75, g2 = 0.75 * (2.0 - s2) * (2.0 - s2) / s2, g3 = 0.75 * (2.0 - s3) * (2.0 - s3) / s3;
+  if (c->kernel == CSPT_KERNEL_POLY5) { g1 = 0.31640625; g2 = 0.0625; g3 = 0.00390625; }
   double S = 2.0 * g1 + 8.0 * g2 + 8.0 * g3;
   P.a1 = (T)(g1 / S); P.a2 = (T)(g2 / S); P.a3 = (T)(g3 / S);
   P.wnorm = (T)(1.0 / ((double)(T)S * (double)P.h * (double)P.h));
@@ -218,12 +220,15 @@ template <class T, int TX, int TY, int CY, int NST, int MINB>
 bool corr_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
   typedef CorrSmem<T, TX, TY, CY, NST> SC;
   const Layout& L = c->L;
-  auto kern = k_corrector_stream<T, TX, TY, CY, NST, MINB>;
+  auto kern0 = k_corrector_stream<T, TX, TY, CY, NST, MINB, 0>;
+  auto kern1 = k_corrector_stream<T, TX, TY, CY, NST, MINB, 1>;
   if (!P) {
     return make_field_map(&c->mapS, field<T>(c, S_ST), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, SC::NF, SC::BX,
                           SC::BY, SC::NF) &&
-           cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, SC::BYTES) == cudaSuccess;
+           cudaFuncSetAttribute(kern0, cudaFuncAttributeMaxDynamicSharedMemorySize, SC::BYTES) == cudaSuccess &&
+           cudaFuncSetAttribute(kern1, cudaFuncAttributeMaxDynamicSharedMemorySize, SC::BYTES) == cudaSuccess;
   }
+  auto kern = c->kernel == CSPT_KERNEL_POLY5 ? kern1 : kern0;
   int gx = (L.nx + 2 + TX - 1) / TX, gy = (L.ny + 2 + TY - 1) / TY;
   int zc = pick_zchunk(gx * gy, L.nz + 2);
   dim3 grid(gx, gy, (L.nz + 2 + zc - 1) / zc);
@@ -474,6 +479,13 @@ int cspt_compute_dt(cspt_ctx* c, double cfl, double* dt_host_out) {
   if (!c->has_state) return CSPT_ESTATE;
   if (c->cuda_error) return CSPT_ECUDA;
   return DISPATCH(c, compute_dt_t)(c, cfl, dt_host_out);
+}
+
+int cspt_set_kernel(cspt_ctx* c, int kernel) {
+  if (!c || (kernel != CSPT_KERNEL_CUBIC_SPLINE && kernel != CSPT_KERNEL_POLY5)) return CSPT_EINVAL;
+  if (kernel != c->kernel) c->has_state = false;      // f = -D[psi] was formed with the other lattice weights
+  c->kernel = kernel;
+  return CSPT_OK;
 }
 
 int cspt_set_limiter(cspt_ctx* c, int limiter) {

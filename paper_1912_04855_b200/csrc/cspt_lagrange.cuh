@@ -196,7 +196,7 @@ struct CorrSmem {
   static_assert((BX * sizeof(T)) % 16 == 0, "box rows must be multiples of 16 bytes");
 };
 
-template <class T, int TX, int TY, int CY, int NST, int MINB>
+template <class T, int TX, int TY, int CY, int NST, int MINB, int KERN>
 __global__ void __launch_bounds__(TX*(TY / CY), MINB)
 k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const DevScalars<T>* __restrict__ sc,
                    const T* __restrict__ U, const T* __restrict__ F, const T* __restrict__ ST, T* __restrict__ UT,
@@ -309,11 +309,17 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
               if (oy < -1 || oy > 1 || (oz == 0 && oy == 0 && ox == 0)) continue;
               const T dx = ei[c][0][ox + 1] - exj, dy = ei[c][1][oy + 1] - eyj, dz = ei[c][2][oz + 1] - ezj;
               const T s = fma(dz, dz, fma(dy, dy, fma(dx, dx, FT::tiny())));
-              T y, q;
-              FT::rsqrt_sqrt(s, y, q);
-              const T g1 = fma((T)-2.25, q, (T)3);
-              const T g2 = fma((T)0.75, q, fma((T)3, y, (T)-3));
-              const T g = FT::lt1(s) ? g1 : (FT::lt4(s) ? g2 : (T)0);
+              T g;
+              if (KERN == 1) {                       // W ~ (1 - q^2/4)^5: g^ = (1 - s/4)^4 on s < 4
+                const T t = fma((T)-0.25, s, (T)1), t2 = t * t;
+                g = FT::lt4(s) ? t2 * t2 : (T)0;
+              } else {                               // cubic spline (G5)
+                T y, q;
+                FT::rsqrt_sqrt(s, y, q);
+                const T g1 = fma((T)-2.25, q, (T)3);
+                const T g2 = fma((T)0.75, q, fma((T)3, y, (T)-3));
+                g = FT::lt1(s) ? g1 : (FT::lt4(s) ? g2 : (T)0);
+              }
               const T w = pj * g;
               sx[c] = fma(w, dx, sx[c]); sy[c] = fma(w, dy, sy[c]); sz[c] = fma(w, dz, sz[c]);
               se[c] = fma(w, fma(wj, dz, fma(vj, dy, uj * dx)), se[c]);

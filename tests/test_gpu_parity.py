@@ -48,13 +48,17 @@ def field_errors(gpu, orc):
     return errs
 
 
-def run_pair(cspt, orc_mod, w, steps, tol, gpu_dtype=None, fields=None, check_dt=True, limiter=0):
+def run_pair(cspt, orc_mod, w, steps, tol, gpu_dtype=None, fields=None, check_dt=True, limiter=0, kernel=0):
     """Steps both sides with the oracle's dt sequence; returns (solver, oracle)."""
     f = fields if fields is not None else w.fields()
     gd = gpu_dtype or w.dtype
     o = make_oracle(orc_mod, w, dtype="f64" if gd == "f32" else w.dtype)
+    if kernel:
+        o.set_kernel(kernel)
     o.set_state(*[np.asarray(a, dtype=np.float64) for a in f] if gd == "f32" else f)
     s = make_solver(cspt, w, dtype=gd)
+    if kernel:
+        s.set_kernel(kernel)       # before set_state: f = -D[psi] uses the kernel's lattice weights
     s.set_state(*f)
     if limiter:
         o.set_limiter(limiter)
@@ -194,6 +198,39 @@ def test_limiter_switch_changes_the_result_and_rejects_unknown_values(cspt, orac
     b.set_limiter(cspt.LIMITER_MINMOD)
     with pytest.raises(cspt.CsptError) as e:
         b.set_limiter(7)
+    assert e.value.code == cspt.EINVAL
+
+
+# ---- the smoothing-kernel switch: W ~ (1 - q^2/4)^5 on both sides ------------------------
+@pytest.mark.parametrize("dims,bc,dtype", [
+    ((40, 37, 21), [0] * 6, "f64"),
+    ((33, 18, 45), [1, 2, 0, 0, 1, 1], "f64"),
+    ((40, 37, 21), [0] * 6, "f32"),
+])
+def test_poly5_kernel_random_smooth(cspt, oracle_mod, dims, bc, dtype):
+    w = wl.random_smooth(*dims, bc=bc, dtype=dtype)
+    run_pair(cspt, oracle_mod, w, 10, TOL64 if dtype == "f64" else TOL32, kernel=cspt.KERNEL_POLY5)
+
+
+def test_poly5_kernel_sod_well_disk(cspt, oracle_mod):
+    run_pair(cspt, oracle_mod, wl.sod(axis=2), 10, TOL64, kernel=cspt.KERNEL_POLY5)
+    run_pair(cspt, oracle_mod, wl.well(n=28, variant="flow"), 10, TOL64, kernel=cspt.KERNEL_POLY5,
+             limiter=cspt.LIMITER_VANLEER)
+    run_pair(cspt, oracle_mod, wl.disk(n=40, dtype="f64"), 10, TOL64, kernel=cspt.KERNEL_POLY5)
+
+
+def test_kernel_switch_discards_the_state_and_rejects_unknown_values(cspt, oracle_mod):
+    w = wl.random_smooth(20, 12, 9)
+    s = make_solver(cspt, w)
+    s.set_state(*w.fields())
+    s.set_kernel(cspt.KERNEL_CUBIC_SPLINE)          # unchanged: the state stays
+    s.step(1e-3)
+    s.set_kernel(cspt.KERNEL_POLY5)                 # changed: f = -D[psi] is stale, the state is discarded
+    with pytest.raises(cspt.CsptError) as e:
+        s.step(1e-3)
+    assert e.value.code == cspt.ESTATE
+    with pytest.raises(cspt.CsptError) as e:
+        s.set_kernel(5)
     assert e.value.code == cspt.EINVAL
 
 
