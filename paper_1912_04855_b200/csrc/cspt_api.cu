@@ -223,8 +223,9 @@ bool corr_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
   auto kern0 = k_corrector_stream<T, TX, TY, CY, NST, MINB, 0>;
   auto kern1 = k_corrector_stream<T, TX, TY, CY, NST, MINB, 1>;
   if (!P) {
-    return make_field_map(&c->mapS, field<T>(c, S_ST), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, SC::NF, SC::BX,
-                          SC::BY, SC::NF) &&
+    // the star group as four pair arrays: inner dimension 2 px elements, 2 fstride elements per array
+    return make_field_map(&c->mapS, field<T>(c, S_ST), (int)sizeof(T), 2 * L.px, L.py, L.pz, 2 * L.fstride, SC::NF,
+                          2 * SC::BX, SC::BY, SC::NF) &&
            cudaFuncSetAttribute(kern0, cudaFuncAttributeMaxDynamicSharedMemorySize, SC::BYTES) == cudaSuccess &&
            cudaFuncSetAttribute(kern1, cudaFuncAttributeMaxDynamicSharedMemorySize, SC::BYTES) == cudaSuccess;
   }

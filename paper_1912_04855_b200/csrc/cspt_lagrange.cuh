@@ -19,8 +19,15 @@
 
 namespace cspt {
 
-// Field order of the star group (slot S_ST): what the predictor hands to the corrector.
-enum StarField { ST_PHI = 0, ST_U, ST_V, ST_W, ST_EX, ST_EY, ST_EZ, ST_E, ST_COUNT };
+// The star group (slot S_ST): what the predictor hands to the corrector.  The eight quantities are stored
+// as four arrays of PAIRS interleaved along x,
+//     (phi*, u*)  (v*, w*)  (eta*_x, eta*_y)  (eta*_z, E*)
+// so that HBM sees four long streams instead of eight and a neighbour particle is four vector loads from
+// shared memory.  Pair array k starts at element k * 2 * fstride; the pair of cell c sits at 2c, 2c+1.
+enum StarPair { SP_PHI_U = 0, SP_V_W, SP_EX_EY, SP_EZ_E, SP_COUNT };
+template <class T> struct Pair;
+template <> struct Pair<double> { typedef double2 type; static __device__ __forceinline__ double2 make(double a, double b) { return make_double2(a, b); } };
+template <> struct Pair<float> { typedef float2 type; static __device__ __forceinline__ float2 make(float a, float b) { return make_float2(a, b); } };
 
 // ---- O1 + O3 + O4: primitives, HFC{predictor}, SUL{predictor} as one z-streaming kernel -------------
 // Eq. (7) with the particles at the cell centres is the lattice operator
@@ -164,9 +171,12 @@ k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* _
       const T qe = rho * ((ui * fq[0] + vi * fq[1]) + wi * fq[2]) - (T)0.5 * pn * (((ui * Sx + vi * Sy) + wi * Sz) + Tt);
       const T mx = Uc[1] + dt * qx, my = Uc[2] + dt * qy, mz = Uc[3] + dt * qz, E = Uc[4] + dt * qe;
       Prim<T> ps = prim_quick<T>(rho, mx, my, mz, E, P.gamma, P.rho_vac);
-      ST[cs] = ps.phi; ST[cs + fs] = ps.u; ST[cs + 2 * fs] = ps.v; ST[cs + 3 * fs] = ps.w;
-      ST[cs + 4 * fs] = he * (ui + ps.u); ST[cs + 5 * fs] = he * (vi + ps.v); ST[cs + 6 * fs] = he * (wi + ps.w);
-      ST[cs + 7 * fs] = E;
+      typedef typename Pair<T>::type V2;
+      V2* st2 = (V2*)ST + cs;                       // pair array k: + k * fs pairs
+      st2[0] = Pair<T>::make(ps.phi, ps.u);
+      st2[fs] = Pair<T>::make(ps.v, ps.w);
+      st2[2 * fs] = Pair<T>::make(he * (ui + ps.u), he * (vi + ps.v));
+      st2[3 * fs] = Pair<T>::make(he * (wi + ps.w), E);
     }
     // particle q: had plane q-1 as its o_z = -1 layer, plane q is its own layer
     acc0[0] = acc1[0] + A0x; acc0[1] = acc1[1] + A0y; acc0[2] = acc1[2]; acc0[3] = acc1[3] + T0;
@@ -181,19 +191,19 @@ k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* _
 
 template <class T, int TX, int TY, int CY, int NST>
 struct CorrSmem {
-  // left x halo: 1 cell is needed; tiles start at cell i = -1 (padded index GX-1 = 3), so HXL = 1
-  // (fp64) / 3 (fp32) puts every box row on a 16-byte boundary in global memory.
-  static constexpr int HXL = sizeof(T) == 8 ? 1 : 3;
-  static constexpr int BX = TX + HXL + 1;
+  // halo 1 in x and y; tiles start at cell i = -1 (padded index GX-1 = 3), the box one cell to the left: pair
+  // index 2, i.e. a 16-byte boundary in global memory in both precisions
+  static constexpr int HXL = 1;
+  static constexpr int BX = TX + 2;
   static constexpr int BY = TY + 2;
-  static constexpr int NF = 7;                                   // phi*, u*, eta* (E* is read directly)
-  static constexpr int PLANE = NF * BY * BX;                     // elements per stage
+  static constexpr int NF = SP_COUNT;                            // pair arrays
+  static constexpr int PLANE = NF * BY * BX * 2;                 // elements per stage
   static constexpr int STAGE = (PLANE * (int)sizeof(T) + 127) / 128 * 128;
   static constexpr int OFF_BAR = NST * STAGE;
   static constexpr int BYTES = OFF_BAR + 64 + 128;               // + slack for the 128-byte alignment
   static constexpr int THREADS = TX * (TY / CY);
   static_assert(TY % CY == 0, "TY must be a multiple of CY");
-  static_assert((BX * sizeof(T)) % 16 == 0, "box rows must be multiples of 16 bytes");
+  static_assert((2 * BX * sizeof(T)) % 16 == 0, "box rows must be multiples of 16 bytes");
 };
 
 template <class T, int TX, int TY, int CY, int NST, int MINB, int KERN>
@@ -226,7 +236,7 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
   auto issue = [&](int q) {              // plane q -> its ring slot
     int s = slot_of(q);
     mbar_expect_tx(&bar[s], TX_BYTES);
-    tma_load_4d(sm + s * S::STAGE, &mapS, &bar[s], i0 + GX - S::HXL, j0 + NG - 1, q + NG, 0);
+    tma_load_4d(sm + s * S::STAGE, &mapS, &bar[s], 2 * (i0 + GX - S::HXL), j0 + NG - 1, q + NG, 0);
   };
   if (tid == 0) {
     for (int q = z0 - 1; q < z0 - 1 + NST && q <= z1; ++q) issue(q);
@@ -246,25 +256,26 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
 
   for (int p = z0; p < z1; ++p) {
     wait_plane(p + 1);
-    const T* pl[3] = {(const T*)(sm + slot_of(p - 1) * S::STAGE), (const T*)(sm + slot_of(p) * S::STAGE),
-                      (const T*)(sm + slot_of(p + 1) * S::STAGE)};
-    auto at = [&](const T* base, int f, int ly, int lx) { return base[(f * S::BY + (ly + 1)) * S::BX + (lx + S::HXL)]; };
+    typedef typename Pair<T>::type V2;
+    const V2* pl[3] = {(const V2*)(sm + slot_of(p - 1) * S::STAGE), (const V2*)(sm + slot_of(p) * S::STAGE),
+                       (const V2*)(sm + slot_of(p + 1) * S::STAGE)};
+    auto at = [&](const V2* base, int k, int ly, int lx) { return base[(k * S::BY + (ly + 1)) * S::BX + (lx + S::HXL)]; };
 
     // own particles
-    T phi_i[CY], ui[CY][3], ei[CY][3][3];        // ei[c][comp][o+1] = eta_i - o
+    T phi_i[CY], ui[CY][3], ei[CY][3][3], Es_i[CY];        // ei[c][comp][o+1] = eta_i - o
     T sx[CY], sy[CY], sz[CY], se[CY];
     bool valid[CY];
 #pragma unroll
     for (int c = 0; c < CY; ++c) {
       int ly = ly0 + c;
       valid[c] = i <= L.nx && (j0 + ly) <= L.ny;
-      phi_i[c] = at(pl[1], ST_PHI, ly, tx);
+      const V2 a0 = at(pl[1], SP_PHI_U, ly, tx), a1 = at(pl[1], SP_V_W, ly, tx);
+      const V2 a2 = at(pl[1], SP_EX_EY, ly, tx), a3 = at(pl[1], SP_EZ_E, ly, tx);
+      phi_i[c] = a0.x; ui[c][0] = a0.y; ui[c][1] = a1.x; ui[c][2] = a1.y;
+      Es_i[c] = a3.y;
+      const T ee[3] = {a2.x, a2.y, a3.x};
 #pragma unroll
-      for (int d = 0; d < 3; ++d) {
-        ui[c][d] = at(pl[1], ST_U + d, ly, tx);
-        T e = at(pl[1], ST_EX + d, ly, tx);
-        ei[c][d][0] = e + (T)1; ei[c][d][1] = e; ei[c][d][2] = e - (T)1;
-      }
+      for (int d = 0; d < 3; ++d) { ei[c][d][0] = ee[d] + (T)1; ei[c][d][1] = ee[d]; ei[c][d][2] = ee[d] - (T)1; }
       sx[c] = sy[c] = sz[c] = se[c] = (T)0;
     }
     bool any = false;
@@ -272,7 +283,7 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
     for (int c = 0; c < CY; ++c) any = any || valid[c];
     // own-cell operands of Eq. (6) straight from global memory, requested before the neighbour loop
     // so that their latency is hidden behind it
-    T own[CY][9];
+    T own[CY][8];
 #pragma unroll
     for (int c = 0; c < CY; ++c) {
       const long long cc = L.idx(valid[c] ? i : 0, valid[c] ? j0 + ly0 + c : 0, p);
@@ -280,13 +291,12 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
       for (int f = 0; f < 5; ++f) own[c][f] = __ldg(U + cc + f * fs);
 #pragma unroll
       for (int f = 0; f < 3; ++f) own[c][5 + f] = __ldg(F + cc + f * fs);
-      own[c][8] = __ldg(ST + cc + (long long)ST_E * fs);
     }
 
     if (any) {
 #pragma unroll
       for (int oz = -1; oz <= 1; ++oz) {
-        const T* sp = pl[oz + 1];
+        const V2* sp = pl[oz + 1];
 #pragma unroll
         for (int r = -1; r <= CY; ++r) {
 #pragma unroll
@@ -300,9 +310,9 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
             }
             if (!used) continue;
             const int ly = ly0 + r, lx = tx + ox;
-            const T pj = at(sp, ST_PHI, ly, lx);
-            const T uj = at(sp, ST_U, ly, lx), vj = at(sp, ST_V, ly, lx), wj = at(sp, ST_W, ly, lx);
-            const T exj = at(sp, ST_EX, ly, lx), eyj = at(sp, ST_EY, ly, lx), ezj = at(sp, ST_EZ, ly, lx);
+            const V2 b0 = at(sp, SP_PHI_U, ly, lx), b1 = at(sp, SP_V_W, ly, lx);
+            const V2 b2 = at(sp, SP_EX_EY, ly, lx), b3 = at(sp, SP_EZ_E, ly, lx);
+            const T pj = b0.x, uj = b0.y, vj = b1.x, wj = b1.y, exj = b2.x, eyj = b2.y, ezj = b3.x;
 #pragma unroll
             for (int c = 0; c < CY; ++c) {
               const int oy = r - c;
@@ -337,7 +347,7 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
       const long long cc = L.idx(i, j, p);
       const T rho = own[c][0], mxn = own[c][1], myn = own[c][2], mzn = own[c][3], En = own[c][4];
       const T fx = own[c][5], fy = own[c][6], fz = own[c][7];
-      const T Es = own[c][8];
+      const T Es = Es_i[c];
       const bool ok = rho > P.rho_vac;
       const T ir = ok ? (T)1 / rho : (T)0;
       const T un = mxn * ir, vn = myn * ir, wn = mzn * ir;
