@@ -219,6 +219,17 @@ def oracle_sample(args, w_full, steps, warmup, n_sample):
     return w, times, cores
 
 
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -238,7 +249,8 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": w.dtype, "data": "synthetic",
         "config": config_of(w_full, max(1, args.gpus)),
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "cpu_model": cpu_model()},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -407,6 +419,7 @@ def run_cspt(args):
         ws, times, cores = oracle_sample(args, w, 3, 0, n_s)
         tot = sum(times)
         line["cpu_baseline"] = {"value": ws.cells * len(times) / tot / 1e6, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "cpu_model": cpu_model(),
                                 "sample": "%s instance %dx%dx%d (%s), 3 steps (compute_dt + step), %d threads; %.1f s"
                                 % (ws.name, ws.nx, ws.ny, ws.nz, ws.dtype, cores, tot)}
     print(json.dumps(line))
