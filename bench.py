@@ -38,8 +38,6 @@ KERNEL_WORDS = {
     "predictor": 5 + 3 + 8,        # fused primitives + predictor: U^n, f -> star group (phi*, u*, eta*, E*)
     "corrector": 8 + 5 + 3 + 7,    # star group, U^n, f -> U~, xi
     "euler": 5 + 4 + 3 + 5,        # U^n, U~, xi -> U^{n+1}
-    "lagrange": 5 + 3 + 7,         # fused predictor+corrector: U^n, f -> U~, xi
-    "step_fused": 5 + 3 + 5,       # fully fused step: U^n, f -> U^{n+1}
     "speed_max": 5,
 }
 

@@ -133,9 +133,17 @@ class Solver:
     def _empty(self, n, dtype=None):
         return [self.torch.empty(self.shape, dtype=dtype or self.tdtype, device=self.device) for _ in range(n)]
 
+    # stream hand-over: tensors arrive from / go to torch's current stream, the library works on self.stream
+    def _before(self):
+        self.stream.wait_stream(self.torch.cuda.current_stream())
+
+    def _after(self):
+        self.torch.cuda.current_stream().wait_stream(self.stream)
+
     # -- the C ABI, same names -----------------------------------------------------------
     def set_state(self, rho, u, v, w, p, psi):
         ts = [self._dev(a) for a in (rho, u, v, w, p, psi)]
+        self._before()
         _check(lib().cspt_set_state(self._h, *[_dptr(t) for t in ts]), "cspt_set_state")
         self.stream.synchronize()      # inputs may be temporaries
 
@@ -167,12 +175,16 @@ class Solver:
 
     def get_state(self):
         out = self._empty(5)
+        self._before()
         _check(lib().cspt_get_state(self._h, *[_dptr(t) for t in out]), "cspt_get_state")
+        self._after()
         return out
 
     def get_conserved(self):
         out = self._empty(5)
+        self._before()
         _check(lib().cspt_get_conserved(self._h, *[_dptr(t) for t in out]), "cspt_get_conserved")
+        self._after()
         return out
 
     def get_conserved_host(self, out):
@@ -182,12 +194,15 @@ class Solver:
 
     def set_conserved(self, rho, mx, my, mz, E):
         ts = [self._dev(a) for a in (rho, mx, my, mz, E)]
+        self._before()
         _check(lib().cspt_set_conserved(self._h, *[_dptr(t) for t in ts]), "cspt_set_conserved")
         self.stream.synchronize()
 
     def get_vacuum_mask(self):
         m = self.torch.empty(self.shape, dtype=self.torch.uint8, device=self.device)
+        self._before()
         _check(lib().cspt_get_vacuum_mask(self._h, _dptr(m)), "cspt_get_vacuum_mask")
+        self._after()
         return m
 
     def launch_count(self):

@@ -241,12 +241,11 @@ bool corr_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
   return true;
 }
 
+// 32 x 8 cells per plane, 2 cells per thread, 4 ring stages, 2 CTAs per SM (224 registers in fp64): the fastest of
+// the tile shapes tried on B200 in both precisions (profiles/r1h.md)
 template <class T>
 bool corr_dispatch(cspt_ctx* c, const Params<T>* P, const T* U) {
-  switch (c->corr_variant) {
-    case 3: return corr_variant<T, 32, 8, 2, 4, 3>(c, P, U);
-    default: return corr_variant<T, 32, 8, 2, 4, 2>(c, P, U);     // fastest on B200 in both precisions
-  }
+  return corr_variant<T, 32, 8, 2, 4, 2>(c, P, U);
 }
 
 template <class T>
@@ -391,7 +390,6 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->stream = (cudaStream_t)cuda_stream;
   carve(c);
   if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
-  c->corr_variant = getenv("CSPT_CORR_VARIANT") ? atoi(getenv("CSPT_CORR_VARIANT")) : 0;   // tuning switch
   c->have_maps = dtype == CSPT_F64 ? make_maps<double>(c) : make_maps<float>(c);
   if (!c->have_maps) { (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }
 

@@ -111,7 +111,6 @@ struct cspt_ctx {
   // TMA views (x, y, z, field) of the two U buffers, of the (U~, xi) group and of the star group
   CUtensorMap mapU[2], mapL, mapS;
   bool have_maps;
-  int corr_variant;         // tuning switch (env CSPT_CORR_VARIANT): corrector tile variant
   int kernel;               // CSPT_KERNEL_*: smoothing kernel W of Eq. (7)
   int limiter;              // CSPT_LIMITER_*: TVD slope of Eq. (8) in the Euler stage
   // per-kernel device timing (cspt_profile_*): event pairs recorded around each launch

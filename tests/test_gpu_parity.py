@@ -281,6 +281,28 @@ def test_host_entry_points_roundtrip(cspt, oracle_mod):
         assert torch.equal(x.cpu(), y)
 
 
+def test_explicit_stream_and_two_solvers_alive(cspt, oracle_mod):
+    """The ctx works on the stream it was given (not only torch's current stream), and two solvers of different
+    precision and size can be interleaved on their own streams."""
+    import torch
+    w1, w2 = wl.random_smooth(24, 20, 19), wl.random_smooth(33, 9, 12, dtype="f32")
+    st1, st2 = torch.cuda.Stream(), torch.cuda.Stream()
+    a = cspt.Solver(w1.nx, w1.ny, w1.nz, w1.h, w1.gamma, w1.bc, cspt.F64, stream=st1)
+    b = cspt.Solver(w2.nx, w2.ny, w2.nz, w2.h, w2.gamma, w2.bc, cspt.F32, stream=st2)
+    ref = make_solver(cspt, w1)
+    a.set_state(*w1.fields())
+    b.set_state(*w2.fields())
+    ref.set_state(*w1.fields())
+    for _ in range(5):
+        a.step_cfl(w1.cfl)
+        b.step_cfl(w2.cfl)
+        ref.step_cfl(w1.cfl)
+    ga, gb = a.get_conserved(), b.get_conserved()   # the binding orders its stream against torch's current one
+    for x, y in zip(ga, ref.get_conserved()):
+        assert torch.equal(x, y)                    # deterministic: same kernels, same result, any stream
+    assert all(bool(torch.isfinite(t).all()) for t in gb)
+
+
 def test_errors(cspt):
     s = cspt.Solver(8, 8, 8, 0.1, 1.4, [0] * 6)
     with pytest.raises(cspt.CsptError) as e:
