@@ -189,6 +189,78 @@ k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* _
 }
 
 
+// ---- fp32, two cells per thread: the neighbour sums of both cells in the two halves of packed f32x2 registers
+// (FFMA2 / FADD2 / FMUL2, sm_100): lane x = own cell 0, lane y = own cell 1.  The fp32 corrector is bound by the
+// instruction issue rate, and one packed evaluation replaces two scalar ones.  Rows 0 and 1 of the thread's
+// neighbourhood serve both cells (the same particle, offsets o_y = r and r - 1); row -1 serves only cell 0 and
+// row 2 only cell 1: those two particles share one packed evaluation.  The self term is evaluated too: its d is
+// exactly 0, so it adds exactly 0.
+template <int KERN>
+__device__ __forceinline__ void pair_eval_f32x2(float2 dx, float2 dy, float2 dz, float2 pj, float2 uj, float2 vj,
+                                                float2 wj, float2& sx, float2& sy, float2& sz, float2& se) {
+  const float2 tiny = make_float2(1e-30f, 1e-30f);
+  const float2 s = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __ffma2_rn(dx, dx, tiny)));
+  float2 g;
+  if (KERN == 1) {
+    const float2 t = __ffma2_rn(make_float2(-0.25f, -0.25f), s, make_float2(1.f, 1.f));
+    const float2 t2 = __fmul2_rn(t, t), t4 = __fmul2_rn(t2, t2);
+    g.x = s.x < 4.f ? t4.x : 0.f;
+    g.y = s.y < 4.f ? t4.y : 0.f;
+  } else {
+    float2 y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y.x) : "f"(s.x));
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y.y) : "f"(s.y));
+    const float2 q = __fmul2_rn(s, y);
+    const float2 g1 = __ffma2_rn(make_float2(-2.25f, -2.25f), q, make_float2(3.f, 3.f));
+    const float2 g2 = __ffma2_rn(make_float2(0.75f, 0.75f), q,
+                                 __ffma2_rn(make_float2(3.f, 3.f), y, make_float2(-3.f, -3.f)));
+    g.x = s.x < 1.f ? g1.x : (s.x < 4.f ? g2.x : 0.f);
+    g.y = s.y < 1.f ? g1.y : (s.y < 4.f ? g2.y : 0.f);
+  }
+  const float2 w = __fmul2_rn(pj, g);
+  sx = __ffma2_rn(w, dx, sx); sy = __ffma2_rn(w, dy, sy); sz = __ffma2_rn(w, dz, sz);
+  se = __ffma2_rn(w, __ffma2_rn(wj, dz, __ffma2_rn(vj, dy, __fmul2_rn(uj, dx))), se);
+}
+
+template <int KERN, class At>
+__device__ __forceinline__ void neighbours_f32x2(const float2* const* pl, At at, int ly0, int tx, const float (*ei)[3][3],
+                                                 float* sx, float* sy, float* sz, float* se) {
+  float2 ex[3], ez[3];
+#pragma unroll
+  for (int o = 0; o < 3; ++o) { ex[o] = make_float2(ei[0][0][o], ei[1][0][o]); ez[o] = make_float2(ei[0][2][o], ei[1][2][o]); }
+  // eta_y - o_y: row r is o_y = r for cell 0 and o_y = r - 1 for cell 1
+  const float2 ey_r0 = make_float2(ei[0][1][1], ei[1][1][0]), ey_r1 = make_float2(ei[0][1][2], ei[1][1][1]);
+  const float2 ey_edge = make_float2(ei[0][1][0], ei[1][1][2]);       // row -1 for cell 0, row 2 for cell 1
+  float2 ax = make_float2(0.f, 0.f), ay = ax, az = ax, ae = ax;
+  auto bc = [](float v) { return make_float2(v, v); };
+#pragma unroll
+  for (int oz = -1; oz <= 1; ++oz) {
+    const float2* sp = pl[oz + 1];
+#pragma unroll
+    for (int ox = -1; ox <= 1; ++ox) {
+      const int lx = tx + ox;
+#pragma unroll
+      for (int r = 0; r <= 1; ++r) {
+        const float2 b0 = at(sp, SP_PHI_U, ly0 + r, lx), b1 = at(sp, SP_V_W, ly0 + r, lx);
+        const float2 b2 = at(sp, SP_EX_EY, ly0 + r, lx), b3 = at(sp, SP_EZ_E, ly0 + r, lx);
+        pair_eval_f32x2<KERN>(__fadd2_rn(ex[ox + 1], bc(-b2.x)), __fadd2_rn(r ? ey_r1 : ey_r0, bc(-b2.y)),
+                              __fadd2_rn(ez[oz + 1], bc(-b3.x)), bc(b0.x), bc(b0.y), bc(b1.x), bc(b1.y), ax, ay, az, ae);
+      }
+      {
+        const float2 a0 = at(sp, SP_PHI_U, ly0 - 1, lx), a1 = at(sp, SP_V_W, ly0 - 1, lx);
+        const float2 a2 = at(sp, SP_EX_EY, ly0 - 1, lx), a3 = at(sp, SP_EZ_E, ly0 - 1, lx);
+        const float2 c0 = at(sp, SP_PHI_U, ly0 + 2, lx), c1 = at(sp, SP_V_W, ly0 + 2, lx);
+        const float2 c2 = at(sp, SP_EX_EY, ly0 + 2, lx), c3 = at(sp, SP_EZ_E, ly0 + 2, lx);
+        pair_eval_f32x2<KERN>(__fadd2_rn(ex[ox + 1], make_float2(-a2.x, -c2.x)),
+                              __fadd2_rn(ey_edge, make_float2(-a2.y, -c2.y)),
+                              __fadd2_rn(ez[oz + 1], make_float2(-a3.x, -c3.x)), make_float2(a0.x, c0.x),
+                              make_float2(a0.y, c0.y), make_float2(a1.x, c1.x), make_float2(a1.y, c1.y), ax, ay, az, ae);
+      }
+    }
+  }
+  sx[0] = ax.x; sx[1] = ax.y; sy[0] = ay.x; sy[1] = ay.y; sz[0] = az.x; sz[1] = az.y; se[0] = ae.x; se[1] = ae.y;
+}
+
 template <class T, int TX, int TY, int CY, int NST>
 struct CorrSmem {
   // halo 1 in x and y; tiles start at cell i = -1 (padded index GX-1 = 3), the box one cell to the left: pair
@@ -293,7 +365,9 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
       for (int f = 0; f < 3; ++f) own[c][5 + f] = __ldg(F + cc + f * fs);
     }
 
-    if (any) {
+    if constexpr (sizeof(T) == 4 && CY == 2) {
+      if (any) neighbours_f32x2<KERN>(pl, at, ly0, tx, ei, sx, sy, sz, se);
+    } else if (any) {
 #pragma unroll
       for (int oz = -1; oz <= 1; ++oz) {
         const V2* sp = pl[oz + 1];
