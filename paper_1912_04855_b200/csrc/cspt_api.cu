@@ -269,7 +269,7 @@ bool make_maps(cspt_ctx* c) {
 }
 
 // primitives + HFC/SUL{predictor} over the extended domain interior(+)2
-constexpr int PTX = 32, PTY = 8;
+constexpr int PTX = 32, PTY = 4;
 template <class T>
 void launch_predictor(cspt_ctx* c, const Params<T>& P, const T* U) {
   const Layout& L = c->L;

@@ -86,7 +86,7 @@ struct EulerSmem {
 };
 
 template <class T, int TX, int TY, int LIM>
-__global__ void __launch_bounds__(TX* TY, sizeof(T) == 4 ? 4 : 2)
+__global__ void __launch_bounds__(TX* TY, (sizeof(T) == 4 ? 1024 : 512) / (TX * TY))
 k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL, Params<T> P,
                const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, T* __restrict__ UN,
                typename Real<T>::bits_t* __restrict__ smax_out, int zchunk) {

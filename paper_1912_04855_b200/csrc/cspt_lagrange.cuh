@@ -63,7 +63,7 @@ struct PredSmem {
 };
 
 template <class T, int TX, int TY>
-__global__ void __launch_bounds__(TX* TY, sizeof(T) == 4 ? 3 : 2)
+__global__ void __launch_bounds__(TX* TY, (sizeof(T) == 4 ? 768 : 512) / (TX * TY))
 k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, const T* __restrict__ F,
                    T* __restrict__ ST, int zchunk) {
   typedef PredSmem<T, TX, TY> S;
