@@ -23,6 +23,13 @@ __device__ __forceinline__ T minmod_fast(T a, T b) {
   T r = fabs(a) < fabs(b) ? a : b;
   return a * b > (T)0 ? r : (T)0;
 }
+// fp64: the sign agreement is tested on the high words (integer pipe instead of a DMUL and a DSETP on the FP64
+// pipe); where a or b is zero the smaller magnitude r is that zero, so the result is the same
+template <>
+__device__ __forceinline__ double minmod_fast<double>(double a, double b) {
+  double r = fabs(a) < fabs(b) ? a : b;
+  return (__double2hiint(a) ^ __double2hiint(b)) >= 0 ? r : 0.0;
+}
 
 // One-sided flux parts of one cell along axis d.  Uc/Um/Up: U^n of the cell and of its -/+
 // neighbours; hf = U^{n+1/2} = (U^n + U~)/2 (G10); xi = xi_d of the cell.
