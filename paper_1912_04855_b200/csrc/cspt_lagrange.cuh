@@ -1,13 +1,14 @@
-// cspt_lagrange.cuh -- Lagrangian stage: HFC{corrector} + SUL{corrector}, Eq. (7) at the displaced
-// particle positions r* and Eq. (6) (readings G1-G9), as a TMA-fed
-// z-streaming kernel.
+// cspt_lagrange.cuh -- Lagrangian stage (readings G1-G9) as two z-streaming kernels:
+//   k_predictor_stream: primitives + HFC{predictor} + SUL{predictor}, Eq. (7) at the cell centres and Eq. (5);
+//   k_corrector_stream: HFC{corrector} + SUL{corrector}, Eq. (7) at the displaced positions r* and Eq. (6).
 //
-// One CTA owns a TX x TY column of cells of the extended domain interior(+)1 (G16) and streams along
-// z.  The seven per-particle quantities of U*, r* that a NEIGHBOUR contributes to Eq. (7)
+// Corrector: one CTA owns a TX x TY column of cells of the extended domain interior(+)1 (G16) and streams
+// along z.  The seven per-particle quantities of U*, r* that a NEIGHBOUR contributes to Eq. (7)
 //     phi*, u*, v*, w*, eta* = xi*/h (3 components)
-// arrive per plane as one TMA box (halo 1 in x/y) in a 4-stage shared-memory ring: planes p-1, p,
-// p+1 are resident while plane p is evaluated and plane p+2 is in flight.  A thread owns CY cells
-// adjacent in y, so that a neighbour particle read from shared memory serves up to CY cells.
+// (and E* of the own cell) arrive per plane as one TMA box of four pair arrays (halo 1 in x/y) in a 4-stage
+// shared-memory ring: planes p-1, p, p+1 are resident while plane p is evaluated and plane p+2 is in flight.
+// A thread owns CY cells adjacent in y, so that a neighbour particle read from shared memory serves up to CY
+// cells; in fp32 the two cells share packed f32x2 arithmetic.
 //
 // Per neighbour (lengths in units of h):  d = (eta_i - o) - eta_j,  s = |d|^2,  y = 1/sqrt(s),
 // q = s y,  g^(q) = -W'(q)/q of the cubic spline (G5):  3 - 2.25 q  (s < 1),
