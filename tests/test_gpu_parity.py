@@ -85,6 +85,7 @@ def run_pair(cspt, orc_mod, w, steps, tol, gpu_dtype=None, fields=None, check_dt
     ((24, 20, 19), [2, 1, 0, 0, 1, 1]),
     ((17, 5, 4), [1, 2, 2, 1, 0, 0]),
     ((5, 1, 3), [0] * 6),
+    ((70, 19, 150), [1, 1, 0, 0, 2, 1]),      # several z chunks (capped at 64 planes), ragged x / y tiles
 ])
 def test_random_smooth_fp64(cspt, oracle_mod, dims, bc):
     w = wl.random_smooth(*dims, bc=bc)
