@@ -131,7 +131,10 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
   const T dt = load_dt(sc);
   const T lam = dt * P.inv_h;
   T Um[5], FPzp[5], acc[5], Utp[5];
-  T smax = 0;
+  // running maximum of the exact speeds seen by this thread, seeded with the global maximum so far (other
+  // CTAs' exact speeds: a lower bound of the final maximum)
+  T smax = Real<T>::from_bits(*(volatile typename Real<T>::bits_t*)smax_out);
+  const T speed_margin = sizeof(T) == 8 ? (T)(1.0 + 1e-12) : (T)(1.0 + 1e-5);
   // U^n of plane z0-2 (own column) for the z slope of plane z0-1
   {
     long long c = L.idx(inside ? i : 0, inside ? j : 0, z0 - 2);
@@ -259,8 +262,14 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
         long long c = L.idx(i, j, p - 1);
 #pragma unroll
         for (int q = 0; q < 5; ++q) UN[c + q * fs] = un[q];
-        T sp = cell_speed_exact<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
-        smax = sp > smax ? sp : smax;
+        // CFL speed of U^{n+1} (G15): exactly rounded, but only for cells whose estimate comes within the
+        // filter margin of a speed already known exactly (this thread's maximum or the global one so far);
+        // the true maximum always passes the filter, so the result is the exact maximum
+        T se = cell_speed_estimate<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
+        if (se * speed_margin >= smax) {
+          T sp = cell_speed_exact<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
+          smax = sp > smax ? sp : smax;
+        }
       }
     }
     if (active) {

@@ -267,6 +267,23 @@ def test_step_cfl_matches_compute_dt_then_step(cspt, oracle_mod):
         assert torch.equal(x, y)
 
 
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_epilogue_speed_filter_keeps_dt_bit_exact(cspt, oracle_mod, dtype):
+    """The Euler stage evaluates the exactly rounded CFL speed only for cells that pass a cheap filter; the
+    maximum must still be the exact one: after every step the device-resident value equals a full exact pass
+    over the same state (set_conserved invalidates the cached maximum), bit for bit."""
+    for w in (wl.random_smooth(70, 19, 150, dtype=dtype, bc=[1, 1, 0, 0, 2, 1]), wl.disk(n=40, dtype=dtype),
+              wl.sedov(n=28, dtype=dtype)):
+        s = make_solver(cspt, w)
+        s.set_state(*w.fields())
+        for _ in range(6):
+            s.step_cfl(w.cfl)
+            dt_epilogue = s.compute_dt(w.cfl)
+            U = s.get_conserved()
+            s.set_conserved(*U)
+            assert s.compute_dt(w.cfl) == dt_epilogue
+
+
 def test_host_entry_points_roundtrip(cspt, oracle_mod):
     import torch
     w = wl.random_smooth(20, 12, 9)
