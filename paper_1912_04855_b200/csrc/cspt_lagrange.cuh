@@ -424,7 +424,7 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
       const T fx = own[c][5], fy = own[c][6], fz = own[c][7];
       const T Es = Es_i[c];
       const bool ok = rho > P.rho_vac;
-      const T ir = ok ? (T)1 / rho : (T)0;
+      const T ir = ok ? FT::rcp(rho) : (T)0;
       const T un = mxn * ir, vn = myn * ir, wn = mzn * ir;
       const T us = ui[c][0], vs = ui[c][1], ws = ui[c][2];
       // U* momentum: rho u* (a vacuum particle has phi = 0, so Q_m = rho f there)
