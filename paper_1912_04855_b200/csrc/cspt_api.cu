@@ -216,12 +216,15 @@ int pick_zchunk(int tiles, int nz) {
 // Corrector variants: tile TX x TY cells per plane, CY cells (adjacent in y) per thread, NST ring
 // stages, MINB resident CTAs per SM asked of the compiler.  P == nullptr: set the kernel up (TMA map of
 // the star group, dynamic shared memory); otherwise launch it.
-template <class T, int TX, int TY, int CY, int NST, int MINB>
+// Corrector: tile TX x TY cells per plane, CY cells (adjacent in y) per thread, NST ring stages, MINB resident
+// CTAs per SM asked of the compiler, XP = 1 when x is periodic (interior columns only; the kernel also writes the ghost columns they wrap onto).
+// P == nullptr: set the kernel up (TMA map of the star group, dynamic shared memory); otherwise launch it.
+template <class T, int TX, int TY, int CY, int NST, int MINB, int XP>
 bool corr_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
-  typedef CorrSmem<T, TX, TY, CY, NST> SC;
+  typedef CorrSmem<T, TX, TY, CY, NST, XP> SC;
   const Layout& L = c->L;
-  auto kern0 = k_corrector_stream<T, TX, TY, CY, NST, MINB, 0>;
-  auto kern1 = k_corrector_stream<T, TX, TY, CY, NST, MINB, 1>;
+  auto kern0 = k_corrector_stream<T, TX, TY, CY, NST, MINB, 0, XP>;
+  auto kern1 = k_corrector_stream<T, TX, TY, CY, NST, MINB, 1, XP>;
   if (!P) {
     // the star group as four pair arrays: inner dimension 2 px elements, 2 fstride elements per array
     return make_field_map(&c->mapS, field<T>(c, S_ST), (int)sizeof(T), 2 * L.px, L.py, L.pz, 2 * L.fstride, SC::NF,
@@ -230,7 +233,8 @@ bool corr_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
            cudaFuncSetAttribute(kern1, cudaFuncAttributeMaxDynamicSharedMemorySize, SC::BYTES) == cudaSuccess;
   }
   auto kern = c->kernel == CSPT_KERNEL_POLY5 ? kern1 : kern0;
-  int gx = (L.nx + 2 + TX - 1) / TX, gy = (L.ny + 2 + TY - 1) / TY;
+  int nxe = XP ? L.nx : L.nx + 2;
+  int gx = (nxe + TX - 1) / TX, gy = (L.ny + 2 + TY - 1) / TY;
   int zc = pick_zchunk(gx * gy, L.nz + 2);
   dim3 grid(gx, gy, (L.nz + 2 + zc - 1) / zc);
   int ps_ = prof_open(c, K_CORRECTOR);
@@ -245,7 +249,8 @@ bool corr_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
 // the tile shapes tried on B200 in both precisions (profiles/r1h.md)
 template <class T>
 bool corr_dispatch(cspt_ctx* c, const Params<T>* P, const T* U) {
-  return corr_variant<T, 32, 8, 2, 4, 2>(c, P, U);
+  return c->bc[0] == CSPT_BC_PERIODIC ? corr_variant<T, 32, 8, 2, 4, 2, 1>(c, P, U)
+                                      : corr_variant<T, 32, 8, 2, 4, 2, 0>(c, P, U);
 }
 
 template <class T>
@@ -273,12 +278,14 @@ constexpr int PTX = 32, PTY = 4;
 template <class T>
 void launch_predictor(cspt_ctx* c, const Params<T>& P, const T* U) {
   const Layout& L = c->L;
-  int gx = (L.nx + 4 + PTX - 1) / PTX, gy = (L.ny + 4 + PTY - 1) / PTY;
+  const bool xp = c->bc[0] == CSPT_BC_PERIODIC;        // periodic x: interior columns only, ghost columns copied
+  int x0 = xp ? 0 : -2, x1 = xp ? L.nx : L.nx + 2;
+  int gx = (x1 - x0 + PTX - 1) / PTX, gy = (L.ny + 4 + PTY - 1) / PTY;
   int zc = pick_zchunk(gx * gy, L.nz + 4);
   dim3 grid(gx, gy, (L.nz + 4 + zc - 1) / zc);
   int ps_ = prof_open(c, K_PREDICTOR);
   k_predictor_stream<T, PTX, PTY><<<grid, PTX * PTY, 0, c->stream>>>(P, scalars<T>(c), U, field<T>(c, S_F),
-                                                                      field<T>(c, S_ST), zc);
+                                                                      field<T>(c, S_ST), zc, x0, x1);
   prof_close(c, ps_);
   c->launches++;
 }

@@ -66,18 +66,18 @@ struct PredSmem {
 template <class T, int TX, int TY>
 __global__ void __launch_bounds__(TX* TY, (sizeof(T) == 4 ? 768 : 512) / (TX * TY))
 k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, const T* __restrict__ F,
-                   T* __restrict__ ST, int zchunk) {
+                   T* __restrict__ ST, int zchunk, int x0, int x1) {      // particle columns [x0, x1)
   typedef PredSmem<T, TX, TY> S;
   __shared__ T sbuf[2][S::PLANE];
   const Layout& L = P.L;
   const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
-  const int i0 = -2 + (int)blockIdx.x * TX, j0 = -2 + (int)blockIdx.y * TY;
+  const int i0 = x0 + (int)blockIdx.x * TX, j0 = -2 + (int)blockIdx.y * TY;
   const int z0 = -2 + (int)blockIdx.z * zchunk, z1 = min(L.nz + 2, z0 + zchunk);   // particle planes [z0, z1)
   const long long fs = L.fstride;
   // own cell: its primitives are needed up to ghost layer 3 (neighbour of the last particle), the
   // particle itself exists up to layer 2; beyond that the index is clamped and the result unused
   const int i = min(i0 + tx, L.nx + 2), j = min(j0 + ty, L.ny + 2);
-  const bool valid = (i0 + tx) <= L.nx + 1 && (j0 + ty) <= L.ny + 1;
+  const bool valid = (i0 + tx) < x1 && (j0 + ty) <= L.ny + 1;
   // halo cell of this thread (tile coordinates -1..TX, -1..TY)
   const bool has_halo = tid < S::NHALO;
   int hx, hy;
@@ -102,6 +102,15 @@ k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* _
     const long long co = c_own + (long long)(z0 - 1) * sz, ch = c_halo + (long long)(z0 - 1) * sz;
 #pragma unroll
     for (int f = 0; f < 5; ++f) { Uo[f] = __ldg(U + co + f * fs); Uh[f] = has_halo ? __ldg(U + ch + f * fs) : (T)0; }
+  }
+  // periodic x (x0 == 0: interior columns only): the ghost columns -2, -1, nx, nx+1 hold what this kernel would
+  // compute there, i.e. the value of the column they wrap onto (same inputs, same arithmetic); woff[g] is the
+  // offset from this thread's particle to ghost column g if it wraps onto the particle, else 0
+  int woff[4];
+#pragma unroll
+  for (int g = 0; g < 4; ++g) {
+    const int xd = g < 2 ? g - 2 : L.nx + (g - 2);
+    woff[g] = (x0 == 0 && ((xd % L.nx) + L.nx) % L.nx == i0 + tx) ? xd - (i0 + tx) : 0;
   }
   T fn[3] = {0, 0, 0};            // force of particle q, requested one iteration before it is needed
   T Uc[5] = {0, 0, 0, 0, 0};      // particle q-1: U^n and primitives
@@ -174,10 +183,15 @@ k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* _
       Prim<T> ps = prim_quick<T>(rho, mx, my, mz, E, P.gamma, P.rho_vac);
       typedef typename Pair<T>::type V2;
       V2* st2 = (V2*)ST + cs;                       // pair array k: + k * fs pairs
-      st2[0] = Pair<T>::make(ps.phi, ps.u);
-      st2[fs] = Pair<T>::make(ps.v, ps.w);
-      st2[2 * fs] = Pair<T>::make(he * (ui + ps.u), he * (vi + ps.v));
-      st2[3 * fs] = Pair<T>::make(he * (wi + ps.w), E);
+      const V2 o0 = Pair<T>::make(ps.phi, ps.u), o1 = Pair<T>::make(ps.v, ps.w);
+      const V2 o2 = Pair<T>::make(he * (ui + ps.u), he * (vi + ps.v)), o3 = Pair<T>::make(he * (wi + ps.w), E);
+      st2[0] = o0; st2[fs] = o1; st2[2 * fs] = o2; st2[3 * fs] = o3;
+#pragma unroll
+      for (int g = 0; g < 4; ++g)
+        if (woff[g]) {                          // periodic x: the ghost column this particle wraps onto
+          V2* w2 = st2 + woff[g];
+          w2[0] = o0; w2[fs] = o1; w2[2 * fs] = o2; w2[3 * fs] = o3;
+        }
     }
     // particle q: had plane q-1 as its o_z = -1 layer, plane q is its own layer
     acc0[0] = acc1[0] + A0x; acc0[1] = acc1[1] + A0y; acc0[2] = acc1[2]; acc0[3] = acc1[3] + T0;
@@ -262,12 +276,14 @@ __device__ __forceinline__ void neighbours_f32x2(const float2* const* pl, At at,
   sx[0] = ax.x; sx[1] = ax.y; sy[0] = ay.x; sy[1] = ay.y; sz[0] = az.x; sz[1] = az.y; se[0] = ae.x; se[1] = ae.y;
 }
 
-template <class T, int TX, int TY, int CY, int NST>
+template <class T, int TX, int TY, int CY, int NST, int XP>
 struct CorrSmem {
-  // halo 1 in x and y; tiles start at cell i = -1 (padded index GX-1 = 3), the box one cell to the left: pair
-  // index 2, i.e. a 16-byte boundary in global memory in both precisions
-  static constexpr int HXL = 1;
-  static constexpr int BX = TX + 2;
+  // halo 1 in x and y.  XP = 0: tiles start at cell i = -1 (padded index GX-1 = 3) and the box one cell to the
+  // left, pair index 2: a 16-byte boundary in global memory in both precisions.  XP = 1 (periodic x, interior
+  // columns only): tiles start at i = 0; in fp32 the box then starts two cells to the left (pair index 2 again).
+  static constexpr int X0 = XP ? 0 : -1;
+  static constexpr int HXL = (XP && sizeof(T) == 4) ? 2 : 1;
+  static constexpr int BX = TX + HXL + ((XP && sizeof(T) == 4) ? 2 : 1);
   static constexpr int BY = TY + 2;
   static constexpr int NF = SP_COUNT;                            // pair arrays
   static constexpr int PLANE = NF * BY * BX * 2;                 // elements per stage
@@ -279,18 +295,18 @@ struct CorrSmem {
   static_assert((2 * BX * sizeof(T)) % 16 == 0, "box rows must be multiples of 16 bytes");
 };
 
-template <class T, int TX, int TY, int CY, int NST, int MINB, int KERN>
+template <class T, int TX, int TY, int CY, int NST, int MINB, int KERN, int XP>
 __global__ void __launch_bounds__(TX*(TY / CY), MINB)
 k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const DevScalars<T>* __restrict__ sc,
                    const T* __restrict__ U, const T* __restrict__ F, const T* __restrict__ ST, T* __restrict__ UT,
                    T* __restrict__ XI, int zchunk) {
-  typedef CorrSmem<T, TX, TY, CY, NST> S;
+  typedef CorrSmem<T, TX, TY, CY, NST, XP> S;
   typedef Fast<T> FT;
   extern __shared__ __align__(128) unsigned char sm[];
   uint64_t* bar = (uint64_t*)(sm + S::OFF_BAR);
   const Layout& L = P.L;
   const int tid = threadIdx.x, tx = tid % TX, tq = tid / TX;
-  const int i0 = -1 + (int)blockIdx.x * TX, j0 = -1 + (int)blockIdx.y * TY;
+  const int i0 = S::X0 + (int)blockIdx.x * TX, j0 = -1 + (int)blockIdx.y * TY;
   // output planes [z0, z1) of the extended domain [-1, nz+1)
   const int z0 = -1 + (int)blockIdx.z * zchunk, z1 = min(L.nz + 1, z0 + zchunk);
   const int i = i0 + tx;
@@ -315,6 +331,14 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
     for (int q = z0 - 1; q < z0 - 1 + NST && q <= z1; ++q) issue(q);
   }
 
+  // periodic x (XP: interior columns only): ghost columns -1 and nx hold the value of the column they wrap
+  // onto; woff[g] = offset from this thread's cell to ghost column g if it wraps onto the cell, else 0
+  int woff[2];
+#pragma unroll
+  for (int g = 0; g < 2; ++g) {
+    const int xd = g ? L.nx : -1;
+    woff[g] = (XP && ((xd % L.nx) + L.nx) % L.nx == i) ? xd - i : 0;
+  }
   const T dt = load_dt(sc);
   const T hdt = (T)0.5 * dt, qdt = (T)0.25 * dt;
   const T pnorm = P.wnorm * P.h;                   // 1 / (S0' h): sums are in units of h
@@ -341,7 +365,7 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
 #pragma unroll
     for (int c = 0; c < CY; ++c) {
       int ly = ly0 + c;
-      valid[c] = i <= L.nx && (j0 + ly) <= L.ny;
+      valid[c] = i < L.nx + (XP ? 0 : 1) && (j0 + ly) <= L.ny;
       const V2 a0 = at(pl[1], SP_PHI_U, ly, tx), a1 = at(pl[1], SP_V_W, ly, tx);
       const V2 a2 = at(pl[1], SP_EX_EY, ly, tx), a3 = at(pl[1], SP_EZ_E, ly, tx);
       phi_i[c] = a0.x; ui[c][0] = a0.y; ui[c][1] = a1.x; ui[c][2] = a1.y;
@@ -441,10 +465,19 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
       const T my = (T)0.5 * (myn + mys) + hdt * qy;
       const T mz = (T)0.5 * (mzn + mzs) + hdt * qz;
       const T E = (T)0.5 * (En + Es) + hdt * qe;
+      const T xo[3] = {(T)0.5 * (hdt * (un + us)) + qdt * (un + mx * ir), (T)0.5 * (hdt * (vn + vs)) + qdt * (vn + my * ir),
+                       (T)0.5 * (hdt * (wn + ws)) + qdt * (wn + mz * ir)};
       UT[cc] = mx; UT[cc + fs] = my; UT[cc + 2 * fs] = mz; UT[cc + 3 * fs] = E;
-      XI[cc] = (T)0.5 * (hdt * (un + us)) + qdt * (un + mx * ir);
-      XI[cc + fs] = (T)0.5 * (hdt * (vn + vs)) + qdt * (vn + my * ir);
-      XI[cc + 2 * fs] = (T)0.5 * (hdt * (wn + ws)) + qdt * (wn + mz * ir);
+      XI[cc] = xo[0]; XI[cc + fs] = xo[1]; XI[cc + 2 * fs] = xo[2];
+      if (XP) {
+#pragma unroll
+        for (int g = 0; g < 2; ++g)
+          if (woff[g]) {                        // periodic x: the ghost column this cell wraps onto
+            const long long cw = cc + woff[g];
+            UT[cw] = mx; UT[cw + fs] = my; UT[cw + 2 * fs] = mz; UT[cw + 3 * fs] = E;
+            XI[cw] = xo[0]; XI[cw + fs] = xo[1]; XI[cw + 2 * fs] = xo[2];
+          }
+      }
     }
 
     __syncthreads();                                 // everyone is done with plane p-1
