@@ -585,6 +585,16 @@ void orc_eval_Q(void* vh, const void* xix, const void* xiy, const void* xiz, voi
 #undef BODY
 }
 
+// Padded U^n (component c = 0..4: rho, mx, my, mz, E) right after the ghost fill O0 of the next step, as a
+// (nz+6, ny+6, nx+6) array, x fastest: lets a test state the boundary rules of reading G16 in its own indexing.
+void orc_get_padded(void* vh, int c, void* out) {
+  Handle* hd = (Handle*)vh;
+  if (c < 0 || c > 4) return;
+#define BODY { o->fill_ghosts_U(false); memcpy(out, o->U[c].data(), o->ncell_pad * sizeof(T)); }
+  DISPATCH(hd, BODY, BODY);
+#undef BODY
+}
+
 // lattice constants (a_f, a_e, a_c, S0') for the closed-form pin
 void orc_lattice_constants(void* vh, double* out4) {
   Handle* hd = (Handle*)vh;

@@ -71,6 +71,8 @@ def _load():
     lib.orc_eval_force.restype = None
     lib.orc_eval_Q.argtypes = [vp] * 8
     lib.orc_eval_Q.restype = None
+    lib.orc_get_padded.argtypes = [vp, ci, vp]
+    lib.orc_get_padded.restype = None
     lib.orc_lattice_constants.argtypes = [vp, ctypes.POINTER(cd)]
     lib.orc_lattice_constants.restype = None
     _lib = lib
@@ -168,6 +170,13 @@ class Oracle:
             keep = [self._in(a) for a in xi]
             xin = [_ptr(a) for a in keep]
         _load().orc_eval_Q(self._h, *xin, *[_ptr(a) for a in out])
+        return out
+
+    def get_padded(self, c):
+        """Component c of U^n with its 3 ghost layers per face as the next step's ghost fill leaves them,
+        shape (nz+6, ny+6, nx+6)."""
+        out = np.empty((self.nz + 6, self.ny + 6, self.nx + 6), dtype=self.np_dtype)
+        _load().orc_get_padded(self._h, int(c), _ptr(out))
         return out
 
     def lattice_constants(self):

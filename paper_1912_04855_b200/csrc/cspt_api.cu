@@ -4,7 +4,6 @@
 #include <stdlib.h>
 #include <string.h>
 
-#include "cspt_step.cuh"
 #include "cspt_euler.cuh"
 #include "cspt_lagrange.cuh"
 

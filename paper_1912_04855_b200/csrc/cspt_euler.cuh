@@ -37,7 +37,7 @@ __device__ __forceinline__ double minmod_fast<double>(double a, double b) {
 template <class T>
 __device__ __forceinline__ T vanleer_fast(T a, T b) {
   T ab = a * b, sum = a + b;
-  bool ok = ab > (T)0 && fabs(sum) > Fast<T>::tiny() * (T)1e20;      // keeps the reciprocal seed normal
+  bool ok = ab > (T)0 && fabs(sum) > (sizeof(T) == 8 ? (T)1e-300 : (T)1e-36);      // keeps the reciprocal seed finite
   T r = ((T)2 * ab) * Fast<T>::rcp(ok ? sum : (T)1);
   return ok ? r : (T)0;
 }
@@ -276,7 +276,7 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
         // CFL speed of U^{n+1} (G15): exactly rounded, but only for cells whose estimate comes within the
         // filter margin of a speed already known exactly (this thread's maximum or the global one so far);
         // the true maximum always passes the filter, so the result is the exact maximum
-        T se = cell_speed_estimate<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
+        T se = cell_speed_upper<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
         if (se * speed_margin >= smax) {
           T sp = cell_speed_exact<T>(un[0], un[1], un[2], un[3], un[4], P.gamma, P.rho_vac);
           smax = sp > smax ? sp : smax;

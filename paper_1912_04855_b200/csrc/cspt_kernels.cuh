@@ -34,20 +34,6 @@ __device__ __forceinline__ Prim<T> prim_exact(T rho, T mx, T my, T mz, T E, T ga
   return q;
 }
 
-// Fast version for the step kernels (contraction allowed; parity is to 1e-11 / 1e-4).
-template <class T>
-__device__ __forceinline__ Prim<T> prim_fast(T rho, T mx, T my, T mz, T E, T gamma, T rho_vac) {
-  Prim<T> q;
-  q.ok = rho > rho_vac;
-  T ir = q.ok ? (T)1 / rho : (T)0;
-  q.u = mx * ir; q.v = my * ir; q.w = mz * ir;
-  T ke2 = (mx * q.u + my * q.v) + mz * q.w;
-  T pp = (gamma - (T)1) * (E - (T)0.5 * ke2);
-  q.p = q.ok ? (pp > (T)0 ? pp : (T)0) : (T)0;
-  q.phi = sqrt((T)2 * q.p);
-  return q;
-}
-
 // ---- fast reciprocal / square roots of the step kernels (parity is to 1e-11 / 1e-4, not bit-exact) ----
 // 1/sqrt(s) and sqrt(s) for s > 0, accurate to rounding level for the type.
 template <class T> struct Fast;
@@ -80,6 +66,7 @@ template <> struct Fast<double> {
   static __device__ __forceinline__ bool lt1(double s) { return __double2hiint(s) < 0x3FF00000; }
   static __device__ __forceinline__ bool lt4(double s) { return __double2hiint(s) < 0x40100000; }
   static __device__ __forceinline__ double tiny() { return 1e-300; }
+  static __device__ __forceinline__ double cancel_eps() { return 1.8e-15; }     // 16 ulp: see cell_speed_upper
 };
 template <> struct Fast<float> {
   static __device__ __forceinline__ void rsqrt_sqrt(float s, float& y, float& t) {
@@ -99,6 +86,7 @@ template <> struct Fast<float> {
   static __device__ __forceinline__ bool lt1(float s) { return s < 1.0f; }
   static __device__ __forceinline__ bool lt4(float s) { return s < 4.0f; }
   static __device__ __forceinline__ float tiny() { return 1e-30f; }
+  static __device__ __forceinline__ float cancel_eps() { return 9.6e-7f; }
 };
 
 // ---- set_state: primitives -> conserved, psi into a scratch field ----
@@ -262,16 +250,20 @@ __device__ __forceinline__ T cell_speed_exact(T rho, T mx, T my, T mz, T E, T ga
   return R::add(cs, m);
 }
 
-// Cheap estimate of the same signal speed (fast reciprocal / square root, relative error of a few ulp in fp64,
-// about 1e-6 in fp32).  Used only as a FILTER: a cell whose estimate lies safely below a speed that is already
-// known exactly cannot be the maximum, so the exactly rounded evaluation is skipped for it.
+// Cheap UPPER BOUND of the same signal speed (fast reciprocal / square root).  Used only as a FILTER: a cell whose
+// bound lies below a speed that is already known exactly cannot be the maximum, so the exactly rounded evaluation
+// is skipped for it.  E - rho|u|^2/2 cancels in cold supersonic cells: the contracted (FMA) evaluation here and
+// the separately rounded one of cell_speed_exact then differ by a few ulp of the OPERANDS (relative eps Mach^2 / 2
+// of the result), so the internal energy is raised by 16 ulp of |E| + rho|u|^2 before the square root; the
+// remaining relative errors (reciprocal and square-root seeds, a few ulp) are covered by the caller's margin.
 template <class T>
-__device__ __forceinline__ T cell_speed_estimate(T rho, T mx, T my, T mz, T E, T gamma, T rho_vac) {
+__device__ __forceinline__ T cell_speed_upper(T rho, T mx, T my, T mz, T E, T gamma, T rho_vac) {
   typedef Fast<T> FT;
   if (!(rho > rho_vac)) return (T)0;
   T ir = FT::rcp(rho);
   T u = mx * ir, v = my * ir, w = mz * ir;
-  T pp = (gamma - (T)1) * (E - (T)0.5 * ((mx * u + my * v) + mz * w));
+  T ke2 = (mx * u + my * v) + mz * w;
+  T pp = (gamma - (T)1) * ((E - (T)0.5 * ke2) + FT::cancel_eps() * (fabs(E) + ke2));
   pp = pp > (T)0 ? pp : (T)0;
   T a = fabs(u), b = fabs(v), c = fabs(w);
   T m = a > b ? a : b;
@@ -332,5 +324,11 @@ __global__ void k_set_dt(DevScalars<T>* sc, T dt) { sc->dt = dt; }
 
 template <class T>
 __global__ void k_reset_smax(DevScalars<T>* sc) { sc->smax_bits = 0; }
+
+template <class T>
+__device__ __forceinline__ T load_dt(const DevScalars<T>* sc) {
+  T dt = sc->dt;
+  return dt < Real<T>::inf() ? dt : (T)0;       // all-vacuum grid: dt = +inf -> identity step
+}
 
 }  // namespace cspt

@@ -1,6 +1,6 @@
 """GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times
-(`cspt_step_cfl`, device-resident dt): sampled windows the oracle can afford (SURVEY.md
-section 8(d)).
+(`cspt_step_cfl`, device-resident dt): sampled 64^3 windows the oracle can afford, 10 steps
+(DESIGN.md section 6).
 
 One full step reaches +-3 cells (readings G16), so after S steps the state inside a window
 depends only on the initial data within 3*S cells of it.  The GPU runs the whole grid S
@@ -25,6 +25,7 @@ pytestmark = pytest.mark.gpu
 TOL64 = 1e-11
 TOL32 = 1e-4
 REACH = 3          # cells per step
+STEPS = 10         # north_star: "after 10 steps"; windows are 64^3 cores padded by 3*10 cells
 
 
 @pytest.fixture(scope="module")
@@ -73,13 +74,15 @@ def window_box(w, lo, size, pad):
     return box
 
 
-def check_windows(cspt, oracle_mod, w, windows, steps, tol, size=(48, 48, 48), limiter=0):
+def check_windows(cspt, oracle_mod, w, windows, steps, tol, size=(64, 64, 64), limiter=0, riemann=0):
     import torch
     dev = torch.device("cuda", torch.cuda.current_device())
     s = cspt.Solver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, cspt.F64 if w.dtype == "f64" else cspt.F32)
     f = device_fields(w, dev)
     s.set_state(*f)
     s.set_limiter(limiter)
+    if riemann:
+        s.set_riemann(riemann)
     del f
     torch.cuda.empty_cache()
     dts = [s.step_cfl(w.cfl, want_dt=True) for _ in range(steps)]
@@ -102,6 +105,8 @@ def check_windows(cspt, oracle_mod, w, windows, steps, tol, size=(48, 48, 48), l
         o = make_oracle(oracle_mod, ww, dtype="f64")
         o.set_state(*[np.asarray(a, dtype=np.float64) for a in fw])
         o.set_limiter(limiter)
+        if riemann:
+            o.set_riemann(riemann)
         for dt in dts:
             o.step(dt)
         ref = o.get_conserved()
@@ -117,7 +122,7 @@ def check_windows(cspt, oracle_mod, w, windows, steps, tol, size=(48, 48, 48), l
     return worst
 
 
-def corner_and_centre_windows(w, size=48):
+def corner_and_centre_windows(w, size=64):
     n = (w.nx, w.ny, w.nz)
     c = tuple(n[d] // 2 - size // 2 for d in range(3))
     return [c, (0, 0, 0), (n[0] - size, n[1] // 3, 0), (n[0] // 5, n[1] - size, n[2] - size)]
@@ -126,24 +131,24 @@ def corner_and_centre_windows(w, size=48):
 def test_cfg2_sedov_128_full_grid(cspt, oracle_mod):
     """128^3 is small enough for the oracle: one window = the whole grid."""
     w = wl.sedov()
-    check_windows(cspt, oracle_mod, w, [(0, 0, 0)], 5, TOL64, size=(128, 128, 128))
+    check_windows(cspt, oracle_mod, w, [(0, 0, 0)], STEPS, TOL64, size=(128, 128, 128))
 
 
 def test_cfg3_well_256_windows(cspt, oracle_mod):
     w = wl.well()
     wins = corner_and_centre_windows(w) + [(0, 100, 100)]          # inflow face
-    check_windows(cspt, oracle_mod, w, wins, 6, TOL64)
+    check_windows(cspt, oracle_mod, w, wins, STEPS, TOL64)
 
 
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_cfg4_turbulence_512_windows(cspt, oracle_mod, dtype):
     w = wl.turbulence(dtype=dtype)
-    check_windows(cspt, oracle_mod, w, corner_and_centre_windows(w), 6, TOL64 if dtype == "f64" else TOL32)
+    check_windows(cspt, oracle_mod, w, corner_and_centre_windows(w), STEPS, TOL64 if dtype == "f64" else TOL32)
 
 
 def test_cfg4_turbulence_512_vanleer_windows(cspt, oracle_mod):
     w = wl.turbulence()
-    check_windows(cspt, oracle_mod, w, corner_and_centre_windows(w)[:2], 6, TOL64, limiter=cspt.LIMITER_VANLEER)
+    check_windows(cspt, oracle_mod, w, corner_and_centre_windows(w)[:2], STEPS, TOL64, limiter=cspt.LIMITER_VANLEER)
 
 
 def test_cfg5_disk_1024_windows(cspt, oracle_mod):
@@ -153,9 +158,9 @@ def test_cfg5_disk_1024_windows(cspt, oracle_mod):
     if free < 156 * 2 ** 30:
         pytest.skip("needs about 150 GiB of free device memory (workspace 124 GB + inputs 26 GB)")
     w = wl.disk()
-    n, sz = w.nx, 48
+    n, sz = w.nx, 64
     wins = [(n // 2 - sz // 2,) * 3,                    # disk centre
             (n // 2 + 200, n // 2 - sz // 2, n // 2 - 10),  # in the disk, off centre
             (n // 2 + int(0.4 * n) - sz // 2, n // 2, n // 2 - sz // 2),   # the gas-vacuum edge R = 0.4 L
             (0, 0, 0)]                                   # vacuum corner with outflow faces
-    check_windows(cspt, oracle_mod, w, wins, 5, TOL32)
+    check_windows(cspt, oracle_mod, w, wins, STEPS, TOL32)

@@ -284,6 +284,28 @@ def test_epilogue_speed_filter_keeps_dt_bit_exact(cspt, oracle_mod, dtype):
             assert s.compute_dt(w.cfl) == dt_epilogue
 
 
+@pytest.mark.parametrize("dtype,mach", [("f32", 1e3), ("f32", 3e3), ("f64", 1e5), ("f64", 3e6)])
+def test_epilogue_speed_filter_cold_hypersonic_stream(cspt, oracle_mod, dtype, mach):
+    """E - rho|u|^2/2 cancels in cold supersonic cells, so a filter with a fixed relative margin
+    could reject the true maximum (from Mach ~ 300 in fp32).  The filter now compares a rigorous upper bound:
+    the device-resident dt of step_cfl must still equal an exact pass over the same state, bit for bit."""
+    nx, ny, nz = 40, 12, 9
+    r = wl.random_smooth(nx, ny, nz, dtype=dtype)
+    rho, u, v, w_, p, psi = [np.asarray(a, dtype=np.float64) for a in r.fields()]
+    cs = math.sqrt(r.gamma)                       # p / rho ~ 1
+    fields = [rho, mach * cs * (1 + 0.02 * u), 0.3 * mach * cs * v, 0.1 * mach * cs * w_, p, 0 * psi]
+    fields = [a.astype(r.np_dtype) for a in fields]
+    s = make_solver(cspt, r)
+    s.set_state(*fields)
+    for _ in range(5):
+        s.step_cfl(r.cfl)
+        dt_epilogue = s.compute_dt(r.cfl)
+        U = s.get_conserved()
+        s.set_conserved(*U)
+        assert s.compute_dt(r.cfl) == dt_epilogue
+        assert all(bool(np.isfinite(t.cpu().numpy()).all()) for t in U)
+
+
 def test_host_entry_points_roundtrip(cspt, oracle_mod):
     import torch
     w = wl.random_smooth(20, 12, 9)
