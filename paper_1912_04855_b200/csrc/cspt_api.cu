@@ -6,6 +6,7 @@
 
 #include "cspt_euler.cuh"
 #include "cspt_lagrange.cuh"
+#include "cspt_corrector.cuh"
 
 using namespace cspt;
 
@@ -252,6 +253,44 @@ bool corr_dispatch(cspt_ctx* c, const Params<T>* P, const T* U) {
                                       : corr_variant<T, 32, 8, 2, 4, 2, 0>(c, P, U);
 }
 
+// Pair-symmetric corrector (cspt_corrector.cuh): strips of two rows, TY rows per CTA, NST ring stages, MINB CTAs per
+// SM, XS = 1: pairs with the neighbouring lanes shared by warp shuffles (31 output columns per tile).
+template <class T, int TY, int NST, int MINB, int XP, int XS>
+bool pair_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
+  typedef PairSmem<T, TY, NST, XS> SC;
+  const Layout& L = c->L;
+  auto kern0 = k_corrector_pairs<T, TY, NST, MINB, 0, XP, XS>;
+  auto kern1 = k_corrector_pairs<T, TY, NST, MINB, 1, XP, XS>;
+  if (!P) {
+    return make_field_map(&c->mapS, field<T>(c, S_ST), (int)sizeof(T), 2 * L.px, L.py, L.pz, 2 * L.fstride, SC::NF,
+                          2 * SC::BX, SC::BY, SC::NF) &&
+           cudaFuncSetAttribute(kern0, cudaFuncAttributeMaxDynamicSharedMemorySize, SC::BYTES) == cudaSuccess &&
+           cudaFuncSetAttribute(kern1, cudaFuncAttributeMaxDynamicSharedMemorySize, SC::BYTES) == cudaSuccess;
+  }
+  auto kern = c->kernel == CSPT_KERNEL_POLY5 ? kern1 : kern0;
+  int nxe = XP ? L.nx : L.nx + 2;
+  int gx = (nxe + SC::TXO - 1) / SC::TXO, gy = (L.ny + 2 + TY - 1) / TY;
+  int zc = pick_zchunk(gx * gy, L.nz + 2);
+  dim3 grid(gx, gy, (L.nz + 2 + zc - 1) / zc);
+  int ps_ = prof_open(c, K_CORRECTOR);
+  kern<<<grid, SC::THREADS, SC::BYTES, c->stream>>>(c->mapS, *P, scalars<T>(c), U, field<T>(c, S_F), field<T>(c, S_UT),
+                                                     field<T>(c, S_XI), zc);
+  prof_close(c, ps_);
+  c->launches++;
+  return true;
+}
+
+template <class T>
+bool corr_select(cspt_ctx* c, const Params<T>* P, const T* U) {
+  const bool xp = c->bc[0] == CSPT_BC_PERIODIC;
+  switch (c->corr_variant) {
+    case 1: return xp ? pair_variant<T, 8, 4, 2, 1, 0>(c, P, U) : pair_variant<T, 8, 4, 2, 0, 0>(c, P, U);
+    case 2: return xp ? pair_variant<T, 8, 4, 2, 1, 1>(c, P, U) : pair_variant<T, 8, 4, 2, 0, 1>(c, P, U);
+    case 3: return xp ? pair_variant<T, 8, 3, 3, 1, 1>(c, P, U) : pair_variant<T, 8, 3, 3, 0, 1>(c, P, U);
+    default: return corr_dispatch<T>(c, P, U);
+  }
+}
+
 template <class T>
 bool make_maps(cspt_ctx* c) {
   const Layout& L = c->L;
@@ -268,7 +307,7 @@ bool make_maps(cspt_ctx* c) {
          cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
              cudaSuccess;
   }
-  ok = ok && corr_dispatch<T>(c, nullptr, nullptr);
+  ok = ok && corr_select<T>(c, nullptr, nullptr);
   return ok;
 }
 
@@ -292,7 +331,7 @@ void launch_predictor(cspt_ctx* c, const Params<T>& P, const T* U) {
 // HFC/SUL{corrector} over the extended domain interior(+)1
 template <class T>
 void launch_corrector(cspt_ctx* c, const Params<T>& P, const T* U) {
-  corr_dispatch<T>(c, &P, U);
+  corr_select<T>(c, &P, U);
 }
 
 template <class T>
@@ -395,6 +434,7 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->ws = workspace; c->ws_bytes = workspace_bytes;
   c->stream = (cudaStream_t)cuda_stream;
   carve(c);
+  if (const char* e = getenv("CSPT_CORR")) c->corr_variant = atoi(e);        // development switch (A/B runs)
   if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
   c->have_maps = dtype == CSPT_F64 ? make_maps<double>(c) : make_maps<float>(c);
   if (!c->have_maps) { (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }
