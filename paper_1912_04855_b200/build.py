@@ -14,7 +14,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcspt.so")
 SOURCES = ["cspt_api.cu"]
-HEADERS = ["cspt_common.cuh", "cspt_kernels.cuh", "cspt_tma.cuh", "cspt_euler.cuh", "cspt_lagrange.cuh", "cspt_corrector.cuh"]
+HEADERS = ["cspt_common.cuh", "cspt_kernels.cuh", "cspt_tma.cuh", "cspt_euler.cuh", "cspt_lagrange.cuh", "cspt_corrector.cuh", "cspt_euler2.cuh"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",

@@ -7,6 +7,7 @@
 #include "cspt_euler.cuh"
 #include "cspt_lagrange.cuh"
 #include "cspt_corrector.cuh"
+#include "cspt_euler2.cuh"
 
 using namespace cspt;
 
@@ -291,8 +292,36 @@ bool corr_select(cspt_ctx* c, const Params<T>* P, const T* U) {
   }
 }
 
+// Euler stage, second layout (cspt_euler2.cuh): TY rows of 32 cells + one helper warp per CTA.
+// P == nullptr: tensor maps and dynamic shared memory; otherwise launch.
+template <class T, int TY, int MINB>
+bool euler2_variant(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
+  typedef Euler2Smem<T, TY> S;
+  const Layout& L = c->L;
+  if (!P) {
+    bool ok = true;
+    for (int b = 0; b < 2; ++b)
+      ok = ok && make_field_map(&c->mapU[b], field<T>(c, b ? S_U1 : S_U0), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 5,
+                                S::BX, S::UY, 5);
+    ok = ok && make_field_map(&c->mapL, field<T>(c, S_UT), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 7, S::BX, S::LY, 7);
+    ok = ok && cudaFuncSetAttribute(k_euler_rows<T, TY, MINB, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) == cudaSuccess;
+    ok = ok && cudaFuncSetAttribute(k_euler_rows<T, TY, MINB, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) == cudaSuccess;
+    return ok;
+  }
+  int gx = (L.nx + S::TX - 1) / S::TX, gy = (L.ny + TY - 1) / TY;
+  int zc = pick_zchunk(gx * gy, L.nz);
+  dim3 grid(gx, gy, (L.nz + zc - 1) / zc);
+  DevScalars<T>* sc = scalars<T>(c);
+  int ps_ = prof_open(c, K_EULER);
+  auto kern = c->limiter == CSPT_LIMITER_VANLEER ? k_euler_rows<T, TY, MINB, 1, 0> : k_euler_rows<T, TY, MINB, 0, 0>;
+  kern<<<grid, S::THREADS, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, *P, sc, U, UN, &sc->smax_bits, zc);
+  prof_close(c, ps_);
+  c->launches++;
+  return true;
+}
+
 template <class T>
-bool make_maps(cspt_ctx* c) {
+bool euler1_setup(cspt_ctx* c) {
   const Layout& L = c->L;
   typedef EulerSmem<T, ETX, EulerTile<T>::TY> S;
   constexpr int ETY = EulerTile<T>::TY;
@@ -307,6 +336,23 @@ bool make_maps(cspt_ctx* c) {
          cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
              cudaSuccess;
   }
+  return ok;
+}
+
+template <class T>
+bool euler_select(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
+  switch (c->euler_variant) {
+    case 1: return euler2_variant<T, 8, 2>(c, P, U, UN);
+    case 2: return euler2_variant<T, 7, 2>(c, P, U, UN);
+    case 3: return euler2_variant<T, 7, 3>(c, P, U, UN);
+    case 4: return euler2_variant<T, 7, 4>(c, P, U, UN);
+    default: return false;
+  }
+}
+
+template <class T>
+bool make_maps(cspt_ctx* c) {
+  bool ok = c->euler_variant ? euler_select<T>(c, nullptr, nullptr, nullptr) : euler1_setup<T>(c);
   ok = ok && corr_select<T>(c, nullptr, nullptr);
   return ok;
 }
@@ -336,6 +382,7 @@ void launch_corrector(cspt_ctx* c, const Params<T>& P, const T* U) {
 
 template <class T>
 void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
+  if (c->euler_variant) { euler_select<T>(c, &P, U, UN); return; }
   typedef EulerSmem<T, ETX, EulerTile<T>::TY> S;
   constexpr int ETY = EulerTile<T>::TY;
   const Layout& L = c->L;
@@ -434,7 +481,13 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->ws = workspace; c->ws_bytes = workspace_bytes;
   c->stream = (cudaStream_t)cuda_stream;
   carve(c);
-  if (const char* e = getenv("CSPT_CORR")) c->corr_variant = atoi(e);        // development switch (A/B runs)
+  // kernel layouts per precision, each the fastest measured on B200 (profiles/r2_kernels.md): fp64 is bound by
+  // the issue slots of its FP64 instructions and runs the pair-symmetric corrector and the row-per-warp Euler
+  // stage; fp32 keeps the packed-f32x2 corrector and the one-thread-per-cell Euler stage at 4 CTAs per SM
+  c->corr_variant = dtype == CSPT_F64 ? 2 : 0;
+  c->euler_variant = dtype == CSPT_F64 ? 2 : 0;
+  if (const char* e = getenv("CSPT_CORR")) c->corr_variant = atoi(e);        // development switches (A/B runs)
+  if (const char* e = getenv("CSPT_EULER")) c->euler_variant = atoi(e);
   if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
   c->have_maps = dtype == CSPT_F64 ? make_maps<double>(c) : make_maps<float>(c);
   if (!c->have_maps) { (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }

@@ -47,27 +47,49 @@ __device__ __forceinline__ T tvd_slope(T a, T b) {
   return LIM == 1 ? vanleer_fast<T>(a, b) : minmod_fast<T>(a, b);
 }
 
+// sign tests on the high word (integer pipe instead of an FP64 compare); a subnormal double counts as zero
+template <class T> __device__ __forceinline__ bool is_pos(T x) { return x > (T)0; }
+template <class T> __device__ __forceinline__ bool is_neg(T x) { return x < (T)0; }
+template <> __device__ __forceinline__ bool is_pos<double>(double x) { return __double2hiint(x) > 0; }
+template <> __device__ __forceinline__ bool is_neg<double>(double x) { return __double2hiint(x) < 0; }
+
 template <class T, int WANT, int LIM>   // WANT bit 0: FP, bit 1: FM
 __device__ __forceinline__ void flux_parts(const Params<T>& P, int d, const T* Uc, const T* Um, const T* Up, const T* hf,
                                            T xi, T* FP, T* FM) {
-  T cP = ((T)0.5 * (P.h - xi)) * P.inv_h;      // (h - xi)/2 * (1/h): slope is minmod(dU)/h (Eq. (8))
-  T cM = ((T)0.5 * (P.h + xi)) * P.inv_h;
+  // (h -+ xi)/2 * (1/h) = 1/2 -+ xi/(2h): the slope of Eq. (8) is limiter(dU)/h
+  const T h2 = (T)0.5 * P.inv_h;
+  const T cP = fma(-h2, xi, (T)0.5), cM = fma(h2, xi, (T)0.5);
   T UL[5], UR[5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) {
     T mm = tvd_slope<T, LIM>(Uc[q] - Um[q], Up[q] - Uc[q]);      // G12
-    if (WANT & 1) UL[q] = hf[q] + cP * mm;
-    if (WANT & 2) UR[q] = hf[q] - cM * mm;
+    if (WANT & 1) UL[q] = fma(cP, mm, hf[q]);
+    if (WANT & 2) UR[q] = fma(-cM, mm, hf[q]);
   }
   if (WANT & 1) {
-    T u = UL[0] > P.rho_vac ? UL[1 + d] * Fast<T>::rcp(UL[0]) : (T)0;       // G9
-    u = u > (T)0 ? u : (T)0;                                   // G13
+    // max(u^L, 0) with u^L = m_d / rho (0 in vacuum, G9)                                                  (G13)
+    T u;
+    if constexpr (sizeof(T) == 8) {            // rho > 0, so the sign is the momentum's: one integer test
+      const bool ok = UL[0] > P.rho_vac && is_pos<T>(UL[1 + d]);
+      const T r = UL[1 + d] * Fast<T>::rcp(ok ? UL[0] : (T)1);
+      u = ok ? r : (T)0;
+    } else {
+      u = UL[0] > P.rho_vac ? UL[1 + d] * Fast<T>::rcp(UL[0]) : (T)0;
+      u = u > (T)0 ? u : (T)0;
+    }
 #pragma unroll
     for (int q = 0; q < 5; ++q) FP[q] = u * UL[q];
   }
   if (WANT & 2) {
-    T u = UR[0] > P.rho_vac ? UR[1 + d] * Fast<T>::rcp(UR[0]) : (T)0;
-    u = u < (T)0 ? u : (T)0;
+    T u;
+    if constexpr (sizeof(T) == 8) {
+      const bool ok = UR[0] > P.rho_vac && is_neg<T>(UR[1 + d]);
+      const T r = UR[1 + d] * Fast<T>::rcp(ok ? UR[0] : (T)1);
+      u = ok ? r : (T)0;
+    } else {
+      u = UR[0] > P.rho_vac ? UR[1 + d] * Fast<T>::rcp(UR[0]) : (T)0;
+      u = u < (T)0 ? u : (T)0;
+    }
 #pragma unroll
     for (int q = 0; q < 5; ++q) FM[q] = u * UR[q];
   }
