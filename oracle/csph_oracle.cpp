@@ -346,7 +346,7 @@ struct Oracle {
   int limiter = 0;
   T slope(T a, T b) const { return limiter == 1 ? vanleer(a, b) : minmod(a, b); }
 
-  // ---- O7: FGC, Eq. (8) + pressureless HLL flux (G10-G13) ----
+  // ---- O7: FGC, Eq. (8) + Riemann flux at the faces (G10-G13) ----
   void fluxes() {
     for (int d = 0; d < 3; ++d) {
       size_t sd = d == 0 ? 1 : d == 1 ? (size_t)p[0] : (size_t)p[0] * p[1];
@@ -370,10 +370,55 @@ struct Oracle {
             }
             T uL = UL[0] > rho_vac ? UL[1 + d] / UL[0] : (T)0;   // G9
             T uR = UR[0] > rho_vac ? UR[1 + d] / UR[0] : (T)0;
-            T up = uL > (T)0 ? uL : (T)0, um = uR < (T)0 ? uR : (T)0;
-            for (int q = 0; q < 5; ++q) F[d][q][cL] = up * UL[q] + um * UR[q];   // G13
+            T Ff[5];
+            riemann_flux(d, UL, UR, uL, uR, Ff);
+            for (int q = 0; q < 5; ++q) F[d][q][cL] = Ff[q];
           }
     }
+  }
+
+  // Approximate Riemann solver at a face ("the approximate methods of Lax-Friedrichs (LF),
+  // Harten-Lax-van Lier (HLL), and the modified Harten-Lax-van Lier method (HLLC) [14]").  The flux vectors of
+  // Eq. (4) are purely advective, F = u U (reading G3): the pressure acts in the Lagrangian stage, so
+  // the Riemann problem of the Euler stage is the one of the pressureless system, whose only signal speeds are
+  // the velocities themselves.  UL, UR: reconstructed states of Eq. (8); uL, uR: their normal velocities (G9).
+  //   riemann 0 (reading G13, the default): HLL with S_L = min(uL,uR), S_R = max(uL,uR), which is
+  //       F = max(uL,0) UL + min(uR,0) UR in all four sign cases;
+  //   riemann 1 (reading G13b): local Lax-Friedrichs (Rusanov), F = (F_L + F_R)/2 - a (UR - UL)/2 with the largest
+  //       local signal speed a = max(|uL|,|uR|) (a global a = h/dt would not vanish for gas at rest);
+  //   riemann 2 (reading G13c): HLLC, Toro [14] section 10.4 with p = 0 and the wave speeds of riemann 0: contact speed
+  //       S* = [rhoR uR (S_R-uR) - rhoL uL (S_L-uL)] / [rhoR (S_R-uR) - rhoL (S_L-uL)], star states
+  //       U*_K = rho_K (S_K-u_K)/(S_K-S*) [1, S* (normal), v_K, w_K (tangential), E_K/rho_K + (S*-u_K) S*],
+  //       F = F_L | F_L + S_L (U*_L - U_L) | F_R + S_R (U*_R - U_R) | F_R.  Between diverging streams the denominator
+  //       vanishes (no mass in the star region) and the flux through the face is zero.
+  int riemann = 0;
+  void riemann_flux(int d, const T* UL, const T* UR, T uL, T uR, T* Ff) const {
+    if (riemann == 1) {
+      T a = std::fabs(uL) > std::fabs(uR) ? std::fabs(uL) : std::fabs(uR);
+      for (int q = 0; q < 5; ++q)
+        Ff[q] = (T)0.5 * (uL * UL[q] + uR * UR[q]) - (T)0.5 * a * (UR[q] - UL[q]);
+      return;
+    }
+    if (riemann == 2) {
+      T SL = uL < uR ? uL : uR, SR = uL < uR ? uR : uL;
+      if (SL >= (T)0) { for (int q = 0; q < 5; ++q) Ff[q] = uL * UL[q]; return; }
+      if (SR <= (T)0) { for (int q = 0; q < 5; ++q) Ff[q] = uR * UR[q]; return; }
+      T den = UR[0] * (SR - uR) - UL[0] * (SL - uL);
+      if (!(den > (T)0)) { for (int q = 0; q < 5; ++q) Ff[q] = (T)0; return; }
+      T Ss = (UR[0] * uR * (SR - uR) - UL[0] * uL * (SL - uL)) / den;
+      const T* UK = Ss >= (T)0 ? UL : UR;
+      T uK = Ss >= (T)0 ? uL : uR, SK = Ss >= (T)0 ? SL : SR;
+      T rs = UK[0] * (SK - uK) / (SK - Ss);
+      T Us[5];
+      Us[0] = rs;
+      for (int q = 1; q < 4; ++q) Us[q] = rs * (UK[q] / UK[0]);
+      Us[1 + d] = rs * Ss;
+      Us[4] = rs * (UK[4] / UK[0] + (Ss - uK) * Ss);
+      for (int q = 0; q < 5; ++q) Ff[q] = uK * UK[q] + SK * (Us[q] - UK[q]);
+      return;
+    }
+    T up = uL > (T)0 ? uL : (T)0, um = uR < (T)0 ? uR : (T)0;
+    for (int q = 0; q < 5; ++q) Ff[q] = up * UL[q] + um * UR[q];   // G13
   }
 
   // ---- O9: CFL time step (silent in the paper; reading G15) ------------------
@@ -488,6 +533,13 @@ void orc_set_limiter(void* vh, int limiter) {
   Handle* hd = (Handle*)vh;
   if (limiter != 0 && limiter != 1) return;
   DISPATCH(hd, o->limiter = limiter, o->limiter = limiter);
+}
+
+// Riemann solver of the Euler stage: 0 = HLL (default), 1 = Lax-Friedrichs, 2 = HLLC; other values are ignored
+void orc_set_riemann(void* vh, int riemann) {
+  Handle* hd = (Handle*)vh;
+  if (riemann < 0 || riemann > 2) return;
+  DISPATCH(hd, o->riemann = riemann, o->riemann = riemann);
 }
 
 void orc_get_conserved(void* vh, void* rho, void* mx, void* my, void* mz, void* E) {

@@ -21,6 +21,7 @@ _LIB_PATH = os.path.join(_HERE, "libcsph_oracle.so")
 F64, F32 = 0, 1
 BC_PERIODIC, BC_OUTFLOW, BC_INFLOW = 0, 1, 2
 LIMITER_MINMOD, LIMITER_VANLEER = 0, 1
+RIEMANN_HLL, RIEMANN_LF, RIEMANN_HLLC = 0, 1, 2
 KERNEL_CUBIC_SPLINE, KERNEL_POLY5 = 0, 1
 
 _lib = None
@@ -55,6 +56,8 @@ def _load():
     lib.orc_compute_dt.restype = cd
     lib.orc_step.argtypes = [vp, cd]
     lib.orc_set_limiter.argtypes = [vp, ci]
+    lib.orc_set_riemann.argtypes = [vp, ci]
+    lib.orc_set_riemann.restype = None
     lib.orc_set_kernel.argtypes = [vp, ci]
     lib.orc_set_kernel.restype = None
     lib.orc_set_limiter.restype = None
@@ -132,6 +135,10 @@ class Oracle:
     def set_limiter(self, limiter):
         """0 = minmod (default, reading G12), 1 = van Leer."""
         _load().orc_set_limiter(self._h, int(limiter))
+
+    def set_riemann(self, riemann):
+        """0 = HLL (default, reading G13), 1 = local Lax-Friedrichs (G13b), 2 = HLLC (G13c)."""
+        _load().orc_set_riemann(self._h, int(riemann))
 
     def step(self, dt):
         _load().orc_step(self._h, float(dt))
