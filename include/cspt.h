@@ -38,6 +38,8 @@ enum { CSPT_F64 = 0, CSPT_F32 = 1 };
 enum { CSPT_BC_PERIODIC = 0, CSPT_BC_OUTFLOW = 1, CSPT_BC_INFLOW = 2 };
 /* TVD slope limiter of Eq. (8): minmod is the default (reading G12) */
 enum { CSPT_LIMITER_MINMOD = 0, CSPT_LIMITER_VANLEER = 1 };
+/* approximate Riemann solver of the Euler stage: HLL is the default (readings G13, G13b, G13c) */
+enum { CSPT_RIEMANN_HLL = 0, CSPT_RIEMANN_LF = 1, CSPT_RIEMANN_HLLC = 2 };
 /* smoothing kernel W of Eq. (7) (PAPER.md:68 leaves it open, :133): the cubic spline is the default (reading G5) */
 enum { CSPT_KERNEL_CUBIC_SPLINE = 0, CSPT_KERNEL_POLY5 = 1 };
 enum { CSPT_OK = 0, CSPT_EINVAL = -1, CSPT_ENOMEM = -2, CSPT_ECUDA = -3, CSPT_ESTATE = -4 };
@@ -86,6 +88,18 @@ int cspt_set_kernel(cspt_ctx*, int kernel);
  * or CSPT_LIMITER_VANLEER (2ab/(a+b) where the one-sided differences a, b agree in sign, else 0).  Takes effect
  * from the next step.  Host-side only, no device work.  EINVAL: null ctx or unknown limiter. */
 int cspt_set_limiter(cspt_ctx*, int limiter);
+
+/* Chooses the approximate Riemann solver that gives the face fluxes F, G, H of Eq. (4) at t_{n+1/2} (PAPER.md:70-72:
+ * "the approximate methods of Lax-Friedrichs (LF), Harten-Lax-van Lier (HLL), and the modified Harten-Lax-van Lier
+ * method (HLLC)").  The flux vectors of Eq. (4) are advective (the pressure acts in the Lagrangian stage), so the
+ * signal speeds are the face velocities u^L, u^R of the states of Eq. (8):
+ *   CSPT_RIEMANN_HLL  (default) S_L = min, S_R = max of (u^L,u^R):  F = max(u^L,0) U^L + min(u^R,0) U^R;
+ *   CSPT_RIEMANN_LF   local Lax-Friedrichs, F = (u^L U^L + u^R U^R)/2 - max(|u^L|,|u^R|) (U^R - U^L)/2;
+ *   CSPT_RIEMANN_HLLC contact speed S* = (rho^L u^L + rho^R u^R)/(rho^L + rho^R) between converging streams, star
+ *                     state of Toro's HLLC with p = 0; equal to HLL at every other face.
+ * Takes effect from the next step.  Host-side only (LF / HLLC move a CSPT_F32 ctx to the kernel layout that
+ * exchanges face states).  EINVAL: null ctx or unknown solver. */
+int cspt_set_riemann(cspt_ctx*, int riemann);
 
 /* One full step U^n -> U^{n+1} with time step dt (Eq. (4)-(8)): ghost fill,
  * HFC/SUL predictor, HFC/SUL corrector, FGC, SUE.

@@ -13,6 +13,7 @@ F64, F32 = 0, 1
 BC_PERIODIC, BC_OUTFLOW, BC_INFLOW = 0, 1, 2
 LIMITER_MINMOD, LIMITER_VANLEER = 0, 1
 KERNEL_CUBIC_SPLINE, KERNEL_POLY5 = 0, 1
+RIEMANN_HLL, RIEMANN_LF, RIEMANN_HLLC = 0, 1, 2
 OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
 
 # every symbol include/cspt.h declares: (name, restype, argtypes)
@@ -26,6 +27,7 @@ SYMBOLS = [
     ("cspt_compute_dt", _ci, [_vp, _cd, _pd]),
     ("cspt_set_kernel", _ci, [_vp, _ci]),
     ("cspt_set_limiter", _ci, [_vp, _ci]),
+    ("cspt_set_riemann", _ci, [_vp, _ci]),
     ("cspt_step", _ci, [_vp, _cd]),
     ("cspt_step_cfl", _ci, [_vp, _cd, _pd]),
     ("cspt_get_state", _ci, [_vp] * 6),
@@ -161,6 +163,9 @@ class Solver:
 
     def set_limiter(self, limiter):
         _check(lib().cspt_set_limiter(self._h, int(limiter)), "cspt_set_limiter")
+
+    def set_riemann(self, riemann):
+        _check(lib().cspt_set_riemann(self._h, int(riemann)), "cspt_set_riemann")
 
     def step(self, dt):
         _check(lib().cspt_step(self._h, float(dt)), "cspt_step")

@@ -294,6 +294,23 @@ bool corr_select(cspt_ctx* c, const Params<T>* P, const T* U) {
 
 // Euler stage, second layout (cspt_euler2.cuh): TY rows of 32 cells + one helper warp per CTA.
 // P == nullptr: tensor maps and dynamic shared memory; otherwise launch.
+template <class T, int TY, int MINB, int LIM, int RIEM>
+bool euler2_kernel(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
+  typedef Euler2Smem<T, TY> S;
+  auto kern = k_euler_rows<T, TY, MINB, LIM, RIEM>;
+  if (!P) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) == cudaSuccess;
+  const Layout& L = c->L;
+  int gx = (L.nx + S::TX - 1) / S::TX, gy = (L.ny + TY - 1) / TY;
+  int zc = pick_zchunk(gx * gy, L.nz);
+  dim3 grid(gx, gy, (L.nz + zc - 1) / zc);
+  DevScalars<T>* sc = scalars<T>(c);
+  int ps_ = prof_open(c, K_EULER);
+  kern<<<grid, S::THREADS, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, *P, sc, U, UN, &sc->smax_bits, zc);
+  prof_close(c, ps_);
+  c->launches++;
+  return true;
+}
+
 template <class T, int TY, int MINB>
 bool euler2_variant(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
   typedef Euler2Smem<T, TY> S;
@@ -304,20 +321,16 @@ bool euler2_variant(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
       ok = ok && make_field_map(&c->mapU[b], field<T>(c, b ? S_U1 : S_U0), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 5,
                                 S::BX, S::UY, 5);
     ok = ok && make_field_map(&c->mapL, field<T>(c, S_UT), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 7, S::BX, S::LY, 7);
-    ok = ok && cudaFuncSetAttribute(k_euler_rows<T, TY, MINB, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) == cudaSuccess;
-    ok = ok && cudaFuncSetAttribute(k_euler_rows<T, TY, MINB, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) == cudaSuccess;
-    return ok;
+    return ok && euler2_kernel<T, TY, MINB, 0, 0>(c, P, U, UN) && euler2_kernel<T, TY, MINB, 1, 0>(c, P, U, UN) &&
+           euler2_kernel<T, TY, MINB, 0, 1>(c, P, U, UN) && euler2_kernel<T, TY, MINB, 1, 1>(c, P, U, UN) &&
+           euler2_kernel<T, TY, MINB, 0, 2>(c, P, U, UN) && euler2_kernel<T, TY, MINB, 1, 2>(c, P, U, UN);
   }
-  int gx = (L.nx + S::TX - 1) / S::TX, gy = (L.ny + TY - 1) / TY;
-  int zc = pick_zchunk(gx * gy, L.nz);
-  dim3 grid(gx, gy, (L.nz + zc - 1) / zc);
-  DevScalars<T>* sc = scalars<T>(c);
-  int ps_ = prof_open(c, K_EULER);
-  auto kern = c->limiter == CSPT_LIMITER_VANLEER ? k_euler_rows<T, TY, MINB, 1, 0> : k_euler_rows<T, TY, MINB, 0, 0>;
-  kern<<<grid, S::THREADS, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, *P, sc, U, UN, &sc->smax_bits, zc);
-  prof_close(c, ps_);
-  c->launches++;
-  return true;
+  const bool vl = c->limiter == CSPT_LIMITER_VANLEER;
+  switch (c->riemann) {
+    case CSPT_RIEMANN_LF: return vl ? euler2_kernel<T, TY, MINB, 1, 1>(c, P, U, UN) : euler2_kernel<T, TY, MINB, 0, 1>(c, P, U, UN);
+    case CSPT_RIEMANN_HLLC: return vl ? euler2_kernel<T, TY, MINB, 1, 2>(c, P, U, UN) : euler2_kernel<T, TY, MINB, 0, 2>(c, P, U, UN);
+    default: return vl ? euler2_kernel<T, TY, MINB, 1, 0>(c, P, U, UN) : euler2_kernel<T, TY, MINB, 0, 0>(c, P, U, UN);
+  }
 }
 
 template <class T>
@@ -589,6 +602,21 @@ int cspt_set_kernel(cspt_ctx* c, int kernel) {
 int cspt_set_limiter(cspt_ctx* c, int limiter) {
   if (!c || (limiter != CSPT_LIMITER_MINMOD && limiter != CSPT_LIMITER_VANLEER)) return CSPT_EINVAL;
   c->limiter = limiter;
+  return CSPT_OK;
+}
+
+int cspt_set_riemann(cspt_ctx* c, int riemann) {
+  if (!c || (riemann != CSPT_RIEMANN_HLL && riemann != CSPT_RIEMANN_LF && riemann != CSPT_RIEMANN_HLLC)) return CSPT_EINVAL;
+  if (c->cuda_error) return CSPT_ECUDA;
+  // the LF and HLLC fluxes need both states at a face: only the row layout of the Euler stage exchanges states, so a
+  // ctx on the cell-per-thread layout (fp32 default) moves to the row layout (new tensor maps, host side only)
+  if (riemann != CSPT_RIEMANN_HLL && c->euler_variant == 0) {
+    c->euler_variant = c->dtype == CSPT_F64 ? 2 : 3;
+    bool ok = c->dtype == CSPT_F64 ? euler_select<double>(c, nullptr, nullptr, nullptr)
+                                   : euler_select<float>(c, nullptr, nullptr, nullptr);
+    if (!ok) { (void)cudaGetLastError(); c->cuda_error = (int)cudaErrorUnknown; return CSPT_ECUDA; }
+  }
+  c->riemann = riemann;
   return CSPT_OK;
 }
 

@@ -113,6 +113,7 @@ struct cspt_ctx {
   bool have_maps;
   int kernel;               // CSPT_KERNEL_*: smoothing kernel W of Eq. (7)
   int limiter;              // CSPT_LIMITER_*: TVD slope of Eq. (8) in the Euler stage
+  int riemann;              // CSPT_RIEMANN_*: flux at the faces of the Euler stage
   int euler_variant;        // 0: one thread per cell with shared-memory flux exchange, 1/2: rows + helper warp (TY = 8 / 7)
   int corr_variant;         // 0: 26-neighbour corrector, 1: pair-symmetric strips, 2: + shared x pairs (warp shuffles)
   // per-kernel device timing (cspt_profile_*): event pairs recorded around each launch

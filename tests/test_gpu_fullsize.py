@@ -151,6 +151,12 @@ def test_cfg4_turbulence_512_vanleer_windows(cspt, oracle_mod):
     check_windows(cspt, oracle_mod, w, corner_and_centre_windows(w)[:2], STEPS, TOL64, limiter=cspt.LIMITER_VANLEER)
 
 
+@pytest.mark.parametrize("riemann", [1, 2])
+def test_cfg4_turbulence_512_riemann_windows(cspt, oracle_mod, riemann):
+    w = wl.turbulence()
+    check_windows(cspt, oracle_mod, w, corner_and_centre_windows(w)[:2], STEPS, TOL64, riemann=riemann)
+
+
 def test_cfg5_disk_1024_windows(cspt, oracle_mod):
     import torch
     torch.cuda.empty_cache()

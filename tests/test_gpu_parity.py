@@ -48,7 +48,7 @@ def field_errors(gpu, orc):
     return errs
 
 
-def run_pair(cspt, orc_mod, w, steps, tol, gpu_dtype=None, fields=None, check_dt=True, limiter=0, kernel=0):
+def run_pair(cspt, orc_mod, w, steps, tol, gpu_dtype=None, fields=None, check_dt=True, limiter=0, kernel=0, riemann=0):
     """Steps both sides with the oracle's dt sequence; returns (solver, oracle)."""
     f = fields if fields is not None else w.fields()
     gd = gpu_dtype or w.dtype
@@ -63,6 +63,9 @@ def run_pair(cspt, orc_mod, w, steps, tol, gpu_dtype=None, fields=None, check_dt
     if limiter:
         o.set_limiter(limiter)
         s.set_limiter(limiter)
+    if riemann:
+        o.set_riemann(riemann)
+        s.set_riemann(riemann)
     if check_dt and gd == "f64":
         assert s.compute_dt(w.cfl) == o.compute_dt(w.cfl)          # bit-exact on the same input
     for n in range(steps):
@@ -199,6 +202,51 @@ def test_limiter_switch_changes_the_result_and_rejects_unknown_values(cspt, orac
     b.set_limiter(cspt.LIMITER_MINMOD)
     with pytest.raises(cspt.CsptError) as e:
         b.set_limiter(7)
+    assert e.value.code == cspt.EINVAL
+
+
+# ---- the Riemann-solver switch: LF and HLLC on both sides ----------------------------
+def _fast(w):
+    """The generic smooth state with three times the velocity: faces where u^L and u^R differ in sign (colliding
+    and diverging streams), which is where the three solvers differ."""
+    rho, u, v, ww, p, psi = w.fields()
+    return (rho, 3 * u, 3 * v, 3 * ww, p, psi)
+
+
+@pytest.mark.parametrize("riemann", [1, 2])
+@pytest.mark.parametrize("dims,bc,dtype", [
+    ((40, 37, 21), [0] * 6, "f64"),
+    ((33, 18, 45), [1, 2, 0, 0, 1, 1], "f64"),
+    ((70, 19, 150), [1, 1, 0, 0, 2, 1], "f64"),
+    ((40, 37, 21), [0] * 6, "f32"),
+])
+def test_riemann_solvers_random_smooth(cspt, oracle_mod, riemann, dims, bc, dtype):
+    w = wl.random_smooth(*dims, bc=bc, dtype=dtype)
+    run_pair(cspt, oracle_mod, w, 10, TOL64 if dtype == "f64" else TOL32, fields=_fast(w), riemann=riemann)
+
+
+@pytest.mark.parametrize("riemann", [1, 2])
+def test_riemann_solvers_sod_disk_well(cspt, oracle_mod, riemann):
+    run_pair(cspt, oracle_mod, wl.sod(axis=1), 10, TOL64, riemann=riemann)
+    run_pair(cspt, oracle_mod, wl.disk(n=40, dtype="f64"), 10, TOL64, riemann=riemann, limiter=cspt.LIMITER_VANLEER)
+    run_pair(cspt, oracle_mod, wl.well(n=28, variant="flow"), 10, TOL64, riemann=riemann)
+    run_pair(cspt, oracle_mod, wl.disk(n=40, dtype="f32"), 10, TOL32, riemann=riemann)
+
+
+def test_riemann_switch_changes_the_result_and_rejects_unknown_values(cspt, oracle_mod):
+    import torch
+    w = wl.random_smooth(20, 12, 9)
+    out = []
+    for r in (cspt.RIEMANN_HLL, cspt.RIEMANN_LF, cspt.RIEMANN_HLLC):
+        s = make_solver(cspt, w)
+        s.set_state(*_fast(w))
+        s.set_riemann(r)
+        for _ in range(3):
+            s.step(2e-3)
+        out.append(s.get_conserved()[0])
+    assert not torch.equal(out[0], out[1]) and not torch.equal(out[0], out[2]) and not torch.equal(out[1], out[2])
+    with pytest.raises(cspt.CsptError) as e:
+        s.set_riemann(3)
     assert e.value.code == cspt.EINVAL
 
 
