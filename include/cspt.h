@@ -111,6 +111,13 @@ int cspt_step(cspt_ctx*, double dt);
  * the call syncs.  A grid that is all vacuum (dt = +inf) is left unchanged. */
 int cspt_step_cfl(cspt_ctx*, double cfl, double* dt_host_out);
 
+/* nsteps steps of cspt_step_cfl, the launches of two consecutive steps replayed from a CUDA
+ * graph so that small grids are not bound by launch latency; bit-identical to a loop of cspt_step_cfl.  The time
+ * steps stay on the device; their sum since cspt_set_state is kept there too and, if t_host_out is not NULL, copied
+ * to *t_host_out (then the call syncs).  nsteps = 0 only reads the time.  With cspt_profile_enable on, the steps
+ * are launched one by one (event pairs cannot be recorded inside a graph).  EINVAL: cfl <= 0, nsteps < 0. */
+int cspt_run_cfl(cspt_ctx*, double cfl, int nsteps, double* t_host_out);
+
 /* Primitives rho,u,v,w,p of the current state (vacuum cells: u = v = w = p = 0).
  * Device pointers; asynchronous. */
 int cspt_get_state(cspt_ctx*, void* rho, void* u, void* v, void* w, void* p);

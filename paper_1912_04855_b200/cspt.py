@@ -30,6 +30,7 @@ SYMBOLS = [
     ("cspt_set_riemann", _ci, [_vp, _ci]),
     ("cspt_step", _ci, [_vp, _cd]),
     ("cspt_step_cfl", _ci, [_vp, _cd, _pd]),
+    ("cspt_run_cfl", _ci, [_vp, _cd, _ci, _pd]),
     ("cspt_get_state", _ci, [_vp] * 6),
     ("cspt_get_conserved", _ci, [_vp] * 6),
     ("cspt_get_conserved_host", _ci, [_vp] * 6),
@@ -176,6 +177,15 @@ class Solver:
             _check(lib().cspt_step_cfl(self._h, float(cfl), ctypes.byref(out)), "cspt_step_cfl")
             return out.value
         _check(lib().cspt_step_cfl(self._h, float(cfl), None), "cspt_step_cfl")
+        return None
+
+    def run_cfl(self, cfl, nsteps, want_time=False):
+        """nsteps CFL-limited steps from a CUDA graph; returns the time since set_state if want_time."""
+        if want_time:
+            out = ctypes.c_double()
+            _check(lib().cspt_run_cfl(self._h, float(cfl), int(nsteps), ctypes.byref(out)), "cspt_run_cfl")
+            return out.value
+        _check(lib().cspt_run_cfl(self._h, float(cfl), int(nsteps), None), "cspt_run_cfl")
         return None
 
     def get_state(self):

@@ -133,6 +133,7 @@ int set_state_t(cspt_ctx* c, const void* rho, const void* u, const void* v, cons
   long long ne = (long long)(c->L.nx + 4) * (c->L.ny + 4) * (c->L.nz + 4);
   LAUNCH(c, K_FORCE, k_force<T>, blocks_for(ne, TPB, STRIDE_CAP), TPB, P, psi_pad, field<T>(c, S_F));
   fill_ghosts<T>(c, U, 5, 1);
+  LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, scalars<T>(c), 1);
   c->cur = 0;
   c->has_state = true;
   c->smax_valid = false;
@@ -172,7 +173,7 @@ void ensure_smax(cspt_ctx* c) {
   if (c->smax_valid) return;
   Params<T> P = make_params<T>(c);
   long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
-  LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, scalars<T>(c));
+  LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, scalars<T>(c), 0);
   LAUNCH(c, K_SPEED_MAX, k_speed_max<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, field<T>(c, c->cur ? S_U1 : S_U0),
          &scalars<T>(c)->smax_bits);
   c->smax_valid = true;
@@ -416,11 +417,9 @@ void run_step(cspt_ctx* c) {
   const Layout& L = c->L;
   T* U = field<T>(c, c->cur ? S_U1 : S_U0);
   T* UN = field<T>(c, c->cur ? S_U0 : S_U1);
-  DevScalars<T>* sc = scalars<T>(c);
   fill_ghosts<T>(c, U, 5, 0);                                                      // O0
   launch_predictor<T>(c, P, U);                                                    // O1, O3, O4
   launch_corrector<T>(c, P, U);                                                    // O5, O6
-  LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, sc);
   launch_euler<T>(c, P, U, UN);                                                  // O7, O8 (+O9 epilogue)
   c->cur ^= 1;
   c->smax_valid = true;
@@ -446,6 +445,81 @@ int step_cfl_t(cspt_ctx* c, double cfl, double* out) {
   rc = cuda_call(c, cudaStreamSynchronize(c->stream));
   if (rc) return rc;
   *out = (double)*hb;
+  return CSPT_OK;
+}
+
+// ---- cspt_run_cfl: n steps of cspt_step_cfl replayed from a CUDA graph ------------------------------------------
+// One graph holds TWO consecutive steps, so that the ping-pong of the U buffers is back where it started; there is
+// one graph per parity of `cur` at entry.  Anything that changes what a step launches drops the graphs.
+void drop_graphs(cspt_ctx* c) {
+  for (int k = 0; k < 2; ++k)
+    if (c->graph[k]) { cudaGraphExecDestroy(c->graph[k]); c->graph[k] = nullptr; }
+}
+
+// The legacy default stream cannot be captured: a ctx created on it captures and replays on a stream of its own, a
+// BLOCKING one, which the default stream orders itself against implicitly.
+cudaStream_t graph_stream(cspt_ctx* c) {
+  if (c->stream) return c->stream;
+  if (!c->gstream && cudaStreamCreate(&c->gstream) != cudaSuccess) { (void)cudaGetLastError(); return nullptr; }
+  return c->gstream;
+}
+
+template <class T>
+int capture_two_steps(cspt_ctx* c, double cfl) {
+  const int k = c->cur;
+  cudaGraph_t g = nullptr;
+  cudaStream_t gs = graph_stream(c), user = c->stream;
+  if (!gs) { c->cuda_error = (int)cudaErrorUnknown; return CSPT_ECUDA; }
+  int rc = cuda_call(c, cudaStreamBeginCapture(gs, cudaStreamCaptureModeThreadLocal));
+  if (rc) return rc;
+  const long long l0 = c->launches;
+  c->stream = gs;
+  for (int s = 0; s < 2; ++s) {
+    LAUNCH(c, K_SCALAR, k_dt_finalize<T>, 1, 1, scalars<T>(c), (T)cfl, (T)c->h);
+    run_step<T>(c);
+  }
+  c->stream = user;
+  c->launches = l0;                                  // counted when the graph is launched
+  cudaError_t e = cudaStreamEndCapture(gs, &g);
+  if (e != cudaSuccess || !g) { (void)cudaGetLastError(); c->cuda_error = (int)(e ? e : cudaErrorUnknown); return CSPT_ECUDA; }
+  e = cudaGraphInstantiate(&c->graph[k], g, 0);
+  cudaGraphDestroy(g);
+  if (e != cudaSuccess) { (void)cudaGetLastError(); c->cuda_error = (int)e; return CSPT_ECUDA; }
+  c->graph_cfl = cfl;
+  return CSPT_OK;
+}
+
+template <class T>
+int run_cfl_t(cspt_ctx* c, double cfl, int nsteps, double* t_out) {
+  ensure_smax<T>(c);
+  int rc = check(c);
+  if (rc) return rc;
+  int left = nsteps;
+  if (!c->prof_on && left >= 2) {                    // event pairs cannot be recorded inside a graph: plain loop then
+    if (c->graph[c->cur] && c->graph_cfl != cfl) drop_graphs(c);
+    if (!c->graph[c->cur]) {
+      rc = capture_two_steps<T>(c, cfl);
+      if (rc) return rc;
+    }
+    const long long per_pair = 2 * 7;                // 3 ghost fills, predictor, corrector, Euler stage, dt
+    for (; left >= 2; left -= 2) {
+      rc = cuda_call(c, cudaGraphLaunch(c->graph[c->cur], graph_stream(c)));
+      if (rc) return rc;
+      c->launches += per_pair;
+    }
+  }
+  for (; left > 0; --left) {
+    LAUNCH(c, K_SCALAR, k_dt_finalize<T>, 1, 1, scalars<T>(c), (T)cfl, (T)c->h);
+    run_step<T>(c);
+  }
+  rc = check(c);
+  if (rc || !t_out) return rc;
+  double* hb = (double*)c->h_pinned;
+  rc = cuda_call(c, cudaMemcpyAsync(hb, &scalars<T>(c)->time, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  if (rc) return rc;
+  rc = cuda_call(c, cudaStreamSynchronize(c->stream));
+  if (rc) return rc;
+  *t_out = *hb;
   return CSPT_OK;
 }
 
@@ -511,6 +585,8 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
 
 void cspt_destroy(cspt_ctx* c) {
   if (!c) return;
+  drop_graphs(c);
+  if (c->gstream) cudaStreamDestroy(c->gstream);
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   for (int i = 0; i < 2 * c->prof_cap; ++i) cudaEventDestroy(c->prof_ev[i]);
   delete[] c->prof_ev;
@@ -594,13 +670,14 @@ int cspt_compute_dt(cspt_ctx* c, double cfl, double* dt_host_out) {
 
 int cspt_set_kernel(cspt_ctx* c, int kernel) {
   if (!c || (kernel != CSPT_KERNEL_CUBIC_SPLINE && kernel != CSPT_KERNEL_POLY5)) return CSPT_EINVAL;
-  if (kernel != c->kernel) c->has_state = false;      // f = -D[psi] was formed with the other lattice weights
+  if (kernel != c->kernel) { c->has_state = false; drop_graphs(c); }     // f = -D[psi] was formed with the other lattice weights
   c->kernel = kernel;
   return CSPT_OK;
 }
 
 int cspt_set_limiter(cspt_ctx* c, int limiter) {
   if (!c || (limiter != CSPT_LIMITER_MINMOD && limiter != CSPT_LIMITER_VANLEER)) return CSPT_EINVAL;
+  if (limiter != c->limiter) drop_graphs(c);
   c->limiter = limiter;
   return CSPT_OK;
 }
@@ -616,6 +693,7 @@ int cspt_set_riemann(cspt_ctx* c, int riemann) {
                                    : euler_select<float>(c, nullptr, nullptr, nullptr);
     if (!ok) { (void)cudaGetLastError(); c->cuda_error = (int)cudaErrorUnknown; return CSPT_ECUDA; }
   }
+  if (riemann != c->riemann) drop_graphs(c);
   c->riemann = riemann;
   return CSPT_OK;
 }
@@ -632,6 +710,13 @@ int cspt_step_cfl(cspt_ctx* c, double cfl, double* dt_host_out) {
   if (!c->has_state) return CSPT_ESTATE;
   if (c->cuda_error) return CSPT_ECUDA;
   return DISPATCH(c, step_cfl_t)(c, cfl, dt_host_out);
+}
+
+int cspt_run_cfl(cspt_ctx* c, double cfl, int nsteps, double* t_host_out) {
+  if (!c || !(cfl > 0) || !isfinite(cfl) || nsteps < 0) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, run_cfl_t)(c, cfl, nsteps, t_host_out);
 }
 
 int cspt_get_state(cspt_ctx* c, void* rho, void* u, void* v, void* w, void* p) {

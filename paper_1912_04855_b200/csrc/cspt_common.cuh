@@ -83,6 +83,7 @@ template <> struct Real<float> {
 template <class T> struct DevScalars {
   T dt;                                  // time step of the step being enqueued
   typename Real<T>::bits_t smax_bits;    // max signal speed, IEEE bits (positive floats order like integers)
+  double time;                           // sum of the time steps taken since cspt_set_state
 };
 
 // Kernel ids for cspt_profile_* (names in cspt_api.cu, same order).
@@ -116,6 +117,10 @@ struct cspt_ctx {
   int riemann;              // CSPT_RIEMANN_*: flux at the faces of the Euler stage
   int euler_variant;        // 0: one thread per cell with shared-memory flux exchange, 1/2: rows + helper warp (TY = 8 / 7)
   int corr_variant;         // 0: 26-neighbour corrector, 1: pair-symmetric strips, 2: + shared x pairs (warp shuffles)
+  // CUDA graphs of two consecutive cspt_step_cfl steps (cspt_run_cfl), one per parity of `cur` at entry
+  cudaGraphExec_t graph[2];
+  cudaStream_t gstream;             // capture / replay stream of a ctx that lives on the legacy default stream
+  double graph_cfl;                 // the CFL number the graphs were captured with
   // per-kernel device timing (cspt_profile_*): event pairs recorded around each launch
   bool prof_on;
   int prof_used;                    // pairs recorded since the last reset

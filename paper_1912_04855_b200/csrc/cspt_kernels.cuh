@@ -311,19 +311,30 @@ __global__ void k_speed_max(Params<T> P, const T* __restrict__ U, typename Real<
   block_max_to_global<T>(smax, out);
 }
 
-// dt = (cfl*h)/smax in T, one rn operation each: identical to the host formula.
+// dt = (cfl*h)/smax in T, one rn operation each: identical to the host formula.  The maximum is consumed here: it is
+// reset for the Euler stage of this step, which leaves the maximum of U^{n+1} behind.
 template <class T>
 __global__ void k_dt_finalize(DevScalars<T>* sc, T cfl, T h) {
   typedef Real<T> R;
   T smax = R::from_bits(sc->smax_bits);
-  sc->dt = smax > (T)0 ? R::div(R::mul(cfl, h), smax) : R::inf();
+  T dt = smax > (T)0 ? R::div(R::mul(cfl, h), smax) : R::inf();
+  sc->dt = dt;
+  sc->smax_bits = 0;
+  if (dt < R::inf()) sc->time += (double)dt;
 }
 
 template <class T>
-__global__ void k_set_dt(DevScalars<T>* sc, T dt) { sc->dt = dt; }
+__global__ void k_set_dt(DevScalars<T>* sc, T dt) {
+  sc->dt = dt;
+  sc->smax_bits = 0;
+  sc->time += (double)dt;
+}
 
 template <class T>
-__global__ void k_reset_smax(DevScalars<T>* sc) { sc->smax_bits = 0; }
+__global__ void k_reset_smax(DevScalars<T>* sc, int reset_time) {
+  sc->smax_bits = 0;
+  if (reset_time) sc->time = 0.0;
+}
 
 template <class T>
 __device__ __forceinline__ T load_dt(const DevScalars<T>* sc) {

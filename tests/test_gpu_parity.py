@@ -315,6 +315,36 @@ def test_step_cfl_matches_compute_dt_then_step(cspt, oracle_mod):
         assert torch.equal(x, y)
 
 
+@pytest.mark.parametrize("dtype,nsteps", [("f64", 7), ("f64", 2), ("f32", 5), ("f64", 1), ("f64", 0)])
+def test_run_cfl_graph_is_bit_identical_to_a_step_cfl_loop(cspt, oracle_mod, dtype, nsteps):
+    """cspt_run_cfl replays two-step CUDA graphs (+ one plain step when nsteps is odd): same kernels, same
+    order, so the state equals a loop of cspt_step_cfl bit for bit and the device-side time is the sum of its dt."""
+    import torch
+    w = wl.random_smooth(33, 18, 45, bc=[1, 2, 0, 0, 1, 1], dtype=dtype)
+    a, b = make_solver(cspt, w), make_solver(cspt, w)
+    a.set_state(*w.fields())
+    b.set_state(*w.fields())
+    t = 0.0
+    for _ in range(nsteps):
+        t += b.step_cfl(w.cfl, want_dt=True)
+    got_t = a.run_cfl(w.cfl, nsteps, want_time=True)
+    assert got_t == t
+    for x, y in zip(a.get_conserved(), b.get_conserved()):
+        assert torch.equal(x, y)
+    # a second call continues from the other parity of the ping-pong and after a setter dropped the graphs
+    a.set_limiter(cspt.LIMITER_VANLEER)
+    b.set_limiter(cspt.LIMITER_VANLEER)
+    a.run_cfl(w.cfl, 3)
+    for _ in range(3):
+        b.step_cfl(w.cfl)
+    a.run_cfl(w.cfl, 4)
+    for _ in range(4):
+        b.step_cfl(w.cfl)
+    for x, y in zip(a.get_conserved(), b.get_conserved()):
+        assert torch.equal(x, y)
+    assert a.launch_count() == b.launch_count()
+
+
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 def test_epilogue_speed_filter_keeps_dt_bit_exact(cspt, oracle_mod, dtype):
     """The Euler stage evaluates the exactly rounded CFL speed only for cells that pass a cheap filter; the
