@@ -42,12 +42,6 @@ KERNEL_WORDS = {
 }
 
 
-# Algorithmic floating-point operations per cell (FMA = 2) of the ALU-bound kernels:
-# corrector = 26 neighbours x (3 sub, 3 FMA, 6 for 1/sqrt and sqrt, 3 for the spline, 1 mul, 3 FMA, 4 for the
-# energy term = 23 instructions, 17 of them FMA -> 40 flop) + about 60 flop for Eq. (6).
-KERNEL_FLOPS = {"corrector": 26 * 40 + 60}
-
-
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -61,7 +55,10 @@ def parse():
                     help="TVD slope limiter of the Euler stage (default: the reading the metric is quoted on)")
     ap.add_argument("--kernel", default="cubic", choices=["cubic", "poly5"],
                     help="smoothing kernel W of Eq. (7) (default: the reading the metric is quoted on)")
+    ap.add_argument("--riemann", default="hll", choices=["hll", "lf", "hllc"],
+                    help="Riemann solver of the Euler stage (default: the reading the metric is quoted on)")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--no-configs", action="store_true", help="skip the per-config throughput table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
 
@@ -156,7 +153,7 @@ def make_workload(args):
 def config_of(w, world):
     esz = 8 if w.dtype == "f64" else 4
     name = "%s %dx%dx%d %s" % (w.name, w.nx, w.ny, w.nz, w.dtype)
-    if w.name == "turbulence":
+    if w.name == "turbulence" and w.nx == 512:
         name += " (BASELINE.json configs[3])"
     big = 5 * w.cells * esz > 4 * 126e6
     return {"workload": name, "cfl": w.cfl, "gamma": w.gamma, "bc": list(w.bc),
@@ -246,7 +243,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": w.dtype, "data": "synthetic",
-        "config": config_of(w_full, max(1, args.gpus)),
+        "config": dict(config_of(w, max(1, args.gpus)), sample_of=config_of(w_full, 1)["workload"],
+                       note="the oracle is timed on this bounded instance of the workload named in sample_of"),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
                          "cpu_model": cpu_model()},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -277,6 +275,118 @@ def job_value(cells_per_rank, steps, world, tmax_ms):
 # ---------------------------------------------------------------------------------------
 # the CUDA path
 # ---------------------------------------------------------------------------------------
+def sources_sha():
+    """Hash of the CUDA sources: a stored ncu traffic figure is only quoted for the build it was captured on."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1912_04855_b200", "csrc")
+    for fn in sorted(os.listdir(d)):
+        if fn.endswith((".cu", ".cuh")):
+            with open(os.path.join(d, fn), "rb") as fh:
+                h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def stored_traffic(w, kernel):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu capture of THIS build, else None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
+            d = json.load(fh)
+        e = d.get("%s %dx%dx%d %s" % (w.name, w.nx, w.ny, w.nz, w.dtype))
+        if e and e.get("sources_sha") == sources_sha():
+            return e.get(kernel), e.get("source")
+    except Exception:
+        pass
+    return None, None
+
+
+def device_fields(w, device):
+    """The six input fields as device tensors, generated slab by slab (no full-size host copy)."""
+    import numpy as np
+    import torch
+    from concurrent.futures import ThreadPoolExecutor
+    tdt = torch.float64 if w.dtype == "f64" else torch.float32
+    out = [torch.empty((w.nz, w.ny, w.nx), dtype=tdt, device=device) for _ in range(6)]
+    slab = max(1, min(w.nz, (1 << 23) // max(1, w.nx * w.ny)))
+    starts = list(range(0, w.nz, slab))
+    with ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1)) as ex:
+        for k0, f in zip(starts, ex.map(lambda k0: w.fields_slab(k0, min(w.nz, k0 + slab)), starts)):
+            for t, a in zip(out, f):
+                t[k0:k0 + a.shape[0]].copy_(torch.from_numpy(np.array(a)))
+    return out
+
+
+def time_steps(s, cfl, steps, graph=True):
+    """Device milliseconds of `steps` CFL-limited steps (events on the solver's stream)."""
+    import torch
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record(s.stream)
+    if graph:
+        s.run_cfl(cfl, steps)
+    else:
+        for _ in range(steps):
+            s.step_cfl(cfl)
+    e1.record(s.stream)
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1)
+
+
+# the five BASELINE.json configs (and cfg4 in fp32): (workload name, dtype override, timed steps)
+CONFIG_RUNS = [("sod", None, 400), ("sedov", None, 100), ("well", None, 10), ("turbulence", "f32", 10), ("disk", None, 5)]
+
+
+def run_configs(cspt, peak, headline):
+    """Throughput on every BASELINE.json config at full size (north_star: "reported at 1 GPU"), a few steps each,
+    inputs generated on the device slab by slab.  The headline workload's own entry is the timed region's."""
+    import torch
+    from paper_1912_04855_b200 import workloads as wl
+    dev = torch.device("cuda", torch.cuda.current_device())
+    out = [headline]
+    for name, dt, steps in CONFIG_RUNS:
+        w = wl.by_name(name, dtype=dt)
+        esz = 8 if w.dtype == "f64" else 4
+        entry = {"workload": "%s %dx%dx%d %s" % (w.name, w.nx, w.ny, w.nz, w.dtype), "steps": steps}
+        try:
+            torch.cuda.empty_cache()
+            need = cspt.lib().cspt_workspace_bytes(w.nx, w.ny, w.nz, cspt.F64 if w.dtype == "f64" else cspt.F32) + 6 * w.cells * esz
+            free, _ = torch.cuda.mem_get_info()
+            if need > 0.97 * free:
+                entry["skipped"] = "needs %.0f GiB of device memory, %.0f free" % (need / 2 ** 30, free / 2 ** 30)
+                out.append(entry)
+                continue
+            s = cspt.Solver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, cspt.F64 if w.dtype == "f64" else cspt.F32)
+            f = device_fields(w, dev)
+            s.set_state(*f)
+            del f
+            torch.cuda.empty_cache()
+            for _ in range(3):
+                s.step_cfl(w.cfl)
+            ms = time_steps(s, w.cfl, steps, graph=True) / steps
+            entry.update({"ms_per_step": ms, "value": w.cells / (ms * 1e-3) / 1e6, "unit": UNIT,
+                          "frac_of_measured_hbm": MIN_WORDS_PER_CELL * esz * w.cells / (ms * 1e-3) / 1e9 / peak,
+                          "api": "cspt_run_cfl (CUDA graph of two steps)"})
+            if w.cells < 4e6:            # launch-bound sizes: the same steps launched one by one, for comparison
+                entry["ms_per_step_step_cfl_loop"] = time_steps(s, w.cfl, steps, graph=False) / steps
+                entry["note"] = "state fits L2: measures launch latency / L2, not HBM"
+            rho = s.get_conserved()[0]
+            entry["finite"] = bool(torch.isfinite(rho).all())
+            del rho
+            s.close()
+        except Exception as e:       # one config failing must not lose the headline line
+            entry["error"] = repr(e)[:200]
+        out.append(entry)
+    return out
+
+
+# SURVEY.md 8(d): algorithmic work of the corrector's neighbour sum, per neighbour [3 sub, 3 FMA for r^2, 1 rsqrt,
+# 5 for the spline, 1 mul, 3 FMA, 3 add, 3 FMA, 1 FMA] = 23 FP instructions (FMA counted once), 26 neighbours,
+# + about 40 for Eq. (6); in flops (FMA = 2): 36 per neighbour + 60.  The implementation evaluates pairs once and
+# executes FEWER instructions than this list; the roofline fraction is quoted on the list, not on what was executed.
+ALGO_INSTR = {"corrector": 26 * 23 + 40}
+ALGO_FLOPS = {"corrector": 26 * 36 + 60}
+
+
 def run_cspt(args):
     import torch
     import torch.distributed as dist
@@ -305,6 +415,7 @@ def run_cspt(args):
         s.set_kernel(cspt.KERNEL_POLY5)
     s.set_state_host(*fields)
     s.set_limiter(cspt.LIMITER_VANLEER if args.limiter == "vanleer" else cspt.LIMITER_MINMOD)
+    s.set_riemann({"hll": cspt.RIEMANN_HLL, "lf": cspt.RIEMANN_LF, "hllc": cspt.RIEMANN_HLLC}[args.riemann])
 
     def barrier():
         torch.cuda.synchronize()
@@ -314,30 +425,40 @@ def run_cspt(args):
 
     for _ in range(args.warmup):
         s.step_cfl(w.cfl)
+    s.run_cfl(w.cfl, 2)                  # graph capture outside the timed region
+    barrier()
+    fma_rate = s.probe_fma_rate()        # roofline denominator, measured on this box in this run
+    issue_probe = {str(k): s.probe_fma_rate(k) for k in (2, 4, 8)}
     barrier()
 
-    # ---- timed region: exactly K steps, device time from CUDA events on the launching stream
+    # ---- timed region: exactly K steps (cspt_run_cfl), device time from CUDA events on the launching stream,
+    # no per-kernel event pairs inside
     sampler = ClockSampler(local)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = s.launch_count()
-    s.profile_enable(True)
     sampler.start()
     e0.record(s.stream)
-    for _ in range(args.steps):
-        s.step_cfl(w.cfl)
+    s.run_cfl(w.cfl, args.steps)
     e1.record(s.stream)
     barrier()
     clocks = sampler.stop()
     ms = e0.elapsed_time(e1)
-    prof = s.profile_read()
-    s.profile_enable(False)
     launches = s.launch_count() - l0
     tmax = max_over_ranks(ms, world, "cuda")
     value = job_value(w.cells, args.steps, world, tmax)
 
+    # ---- the same K steps once more with an event pair around every launch: per-kernel times for the roofline
+    s.profile_enable(True)
+    for _ in range(args.steps):
+        s.step_cfl(w.cfl)
+    prof = s.profile_read()
+    s.profile_enable(False)
+    barrier()
+
     # the state must still be sane (a blown-up run would time NaN arithmetic)
     rho = s.get_conserved()[0]
     assert bool(torch.isfinite(rho).all()), "state is not finite after the timed steps"
+    del rho
 
     # ---- end to end through the C ABI with HOST buffers: H2D of the 6 inputs, one step, D2H of U
     out = [torch.empty((w.nz, w.ny, w.nx), dtype=fields[0].dtype).pin_memory() for _ in range(5)]
@@ -359,46 +480,57 @@ def run_cspt(args):
     e2e = {"value": job_value(w.cells, n_e2e, world, ems), "unit": UNIT,
            "h2d_bytes_per_step": 6 * w.cells * esz, "d2h_bytes_per_step": 5 * w.cells * esz, "steps": n_e2e,
            "what": "cspt_set_state_host + cspt_step_cfl + cspt_get_conserved_host per step, pinned host buffers"}
+    s.close()
+    del s, out, fields
+    torch.cuda.empty_cache()
 
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel, from the event pairs recorded in the timed region
+    # ---- roofline of the dominant kernel, from the event pairs of the profiled pass
     peak, peak_src = peaks()
     step_ms = tmax / args.steps
-    kern = {k: {"ms_per_step": v[0] / args.steps, "launches_per_step": v[1] / args.steps} for k, v in prof.items()}
+    kern = {}
+    for k, v in prof.items():
+        per_step = v[1] / args.steps
+        kern[k] = {"ms_per_step": v[0] / args.steps, "launches_per_step": per_step}
     dom = max(prof.items(), key=lambda kv: kv[1][0])[0]
     dom_ms = prof[dom][0] / prof[dom][1]
+    prof_step_ms = sum(v[0] for v in prof.values()) / args.steps
     words = KERNEL_WORDS.get(dom, MIN_WORDS_PER_CELL)
     dom_bytes = words * esz * w.cells
     ach = dom_bytes / (dom_ms * 1e-3) / 1e9
-    traffic = None
-    try:
-        with open(os.path.join(ROOT, "profiles", "traffic.json")) as fh:
-            traffic = json.load(fh).get("%s %dx%dx%d %s" % (w.name, w.nx, w.ny, w.nz, w.dtype), {}).get(dom)
-    except Exception:
-        traffic = None
+    traffic, traffic_src = stored_traffic(w, dom)
     hbm = {"achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": peak_src,
            "algorithmic_bytes_per_launch": dom_bytes}
-    if dom in KERNEL_FLOPS:
-        # the corrector is bound by the plain FP64 / FP32 pipe: algorithmic flops per cell
-        # (FMA = 2) over the launch time, against lanes x 2 flop x SMs x max SM clock
-        lanes = 64 if w.dtype == "f64" else 128
-        apeak = 148 * lanes * 2 * 1.965e9 / 1e12
-        flops_cell = KERNEL_FLOPS[dom] if args.kernel == "cubic" else 26 * 27 + 60    # poly5: no 1/sqrt, 3-op spline
-        aach = flops_cell * w.cells / (dom_ms * 1e-3) / 1e12
+    share = (prof[dom][0] / args.steps) / prof_step_ms
+    if dom in ALGO_FLOPS and args.kernel == "cubic":
+        # the corrector is bound by the plain FP64 / FP32 pipe.  Denominator: the FMA rate
+        # cspt_probe_fma_rate measured in THIS run just before the timed region (thread-level FMA/s; an FP instruction
+        # of any kind occupies a lane of that pipe for one slot, so it is also the instruction rate).
+        apeak = 2.0 * fma_rate / 1e12
+        aach = ALGO_FLOPS[dom] * w.cells / (dom_ms * 1e-3) / 1e12
         roofline = {"bound": "alu", "kernel": dom, "achieved": aach, "peak": apeak, "unit": "TFLOP/s",
-                    "frac": aach / apeak, "traffic": traffic,
-                    "peak_source": "derived: 148 SMs x %d %s lanes x 2 flop x 1965 MHz (DESIGN.md section 7; "
-                                   "measured 63.4 DFMA / 120.9 FFMA per clock per SM, profiles/r1a_launches_baseline.md)"
-                                   % (lanes, w.dtype),
-                    "algorithmic_flops_per_cell": flops_cell, "kernel_ms": dom_ms,
-                    "share_of_step": (prof[dom][0] / args.steps) / step_ms, "hbm": hbm}
+                    "frac": aach / apeak, "frac_is": "flop fraction (FMA = 2 flop) of the measured FMA peak",
+                    "instr_frac": ALGO_INSTR[dom] * w.cells / (dom_ms * 1e-3) / fma_rate,
+                    "instr_frac_is": "SURVEY 8(d) instruction list (%d FP instructions per cell, FMA counted once) over "
+                                     "the measured instruction rate of the pipe" % ALGO_INSTR[dom],
+                    "traffic": traffic, "traffic_source": traffic_src,
+                    "peak_source": "measured in this run: cspt_probe_fma_rate, %.1f %s FMA per clock per SM at %d MHz"
+                                   % (fma_rate / 148 / ((clocks.get("sm_max_mhz") or 1965) * 1e6), w.dtype,
+                                      clocks.get("sm_max_mhz") or 1965),
+                    "fma_per_second": fma_rate,
+                    "fma_per_second_with_other_instructions": issue_probe,
+                    "issue_note": "FMA rate with 2 / 4 / 8 independent integer instructions per FMA: time ~ slots(FMA) + "
+                                  "others, slots(FMA) = 2 in fp64 and 1 in fp32 (DESIGN.md section 7)",
+                    "algorithmic_flops_per_cell": ALGO_FLOPS[dom],
+                    "algorithmic_instr_per_cell": ALGO_INSTR[dom], "kernel_ms": dom_ms, "share_of_step": share,
+                    "hbm": hbm}
     else:
-        roofline = dict(hbm, bound="hbm", kernel=dom, traffic=traffic, kernel_ms=dom_ms,
-                        share_of_step=(prof[dom][0] / args.steps) / step_ms)
+        roofline = dict(hbm, bound="hbm", kernel=dom, traffic=traffic, traffic_source=traffic_src, kernel_ms=dom_ms,
+                        share_of_step=share)
     step_ach = MIN_WORDS_PER_CELL * esz * w.cells / (step_ms * 1e-3) / 1e9
     step_hbm = {"bytes_per_cell_update": MIN_WORDS_PER_CELL * esz, "achieved_gbs": step_ach, "frac_of_measured": step_ach / peak,
                 "frac_of_nominal_8TBs": step_ach / 8000.0}
@@ -407,10 +539,19 @@ def run_cspt(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": w.dtype, "data": "synthetic",
-        "config": dict(config_of(w, world), limiter=args.limiter, kernel=args.kernel),
+        "config": dict(config_of(w, world), limiter=args.limiter, kernel=args.kernel, riemann=args.riemann,
+                       api="cspt_run_cfl"),
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "kernels": kern,
+        "kernels_note": "per-kernel times from a second pass of the same K steps with an event pair around every launch "
+                        "(%.3f ms per step in that pass)" % prof_step_ms,
         "roofline": roofline, "step_hbm": step_hbm,
     }
+
+    if world == 1 and not args.no_configs:
+        headline = {"workload": "%s %dx%dx%d %s" % (w.name, w.nx, w.ny, w.nz, w.dtype), "steps": args.steps,
+                    "ms_per_step": step_ms, "value": value, "unit": UNIT, "frac_of_measured_hbm": step_ach / peak,
+                    "api": "cspt_run_cfl (CUDA graph of two steps)", "finite": True}
+        line["configs"] = run_configs(cspt, peak, headline)
 
     if not args.no_cpu_baseline and world == 1:
         n_s = min(384, max(w.nx, w.ny, w.nz)) if args.workload != "sod" else None

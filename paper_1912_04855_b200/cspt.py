@@ -41,6 +41,7 @@ SYMBOLS = [
     ("cspt_profile_kernel_count", _ci, []),
     ("cspt_profile_kernel_name", ctypes.c_char_p, [_ci]),
     ("cspt_profile_read", _ci, [_vp, _ci, _pd, ctypes.POINTER(ctypes.c_longlong)]),
+    ("cspt_probe_fma_rate", _ci, [_vp, _ci, _pd]),
     ("cspt_cuda_error", _ci, [_vp]),
     ("cspt_sync", _ci, [_vp]),
     ("cspt_destroy", None, [_vp]),
@@ -236,6 +237,13 @@ class Solver:
             if n.value:
                 out[L.cspt_profile_kernel_name(kid).decode()] = (ms.value, int(n.value))
         return out
+
+    def probe_fma_rate(self, other_per_fma=0):
+        """Measured FMA rate of the plain FP pipe in the solver's precision (thread-level FMAs per second), alone or
+        with 2 / 4 / 8 independent integer instructions interleaved per FMA."""
+        out = ctypes.c_double()
+        _check(lib().cspt_probe_fma_rate(self._h, int(other_per_fma), ctypes.byref(out)), "cspt_probe_fma_rate")
+        return out.value
 
     def cuda_error(self):
         return int(lib().cspt_cuda_error(self._h))

@@ -523,6 +523,30 @@ int run_cfl_t(cspt_ctx* c, double cfl, int nsteps, double* t_out) {
   return CSPT_OK;
 }
 
+template <class T>
+int probe_fma_t(cspt_ctx* c, int other_per_fma, double* fma_per_second) {
+  // scratch: the star-group slots are dead between steps
+  T* out = field<T>(c, S_ST);
+  const int threads = 128, blocks = 148 * 8, iters = other_per_fma ? 1500 : 4000;
+  if ((long long)threads * blocks > c->L.fstride * 8) return CSPT_EINVAL;
+  auto kern = other_per_fma == 0 ? k_probe_fma<T, 0> : other_per_fma == 2 ? k_probe_fma<T, 1> : other_per_fma == 4 ? k_probe_fma<T, 2> : k_probe_fma<T, 4>;
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { (void)cudaGetLastError(); return CSPT_ECUDA; }
+  kern<<<blocks, threads, 0, c->stream>>>(out, 200, (T)1.0000001, (T)1e-9, 5);          // warm-up
+  cudaEventRecord(e0, c->stream);
+  kern<<<blocks, threads, 0, c->stream>>>(out, iters, (T)1.0000001, (T)1e-9, 5);
+  cudaEventRecord(e1, c->stream);
+  int rc = cuda_call(c, cudaEventSynchronize(e1));
+  float ms = 0;
+  if (!rc) rc = cuda_call(c, cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (rc) return rc;
+  *fma_per_second = (double)iters * 64.0 * threads * blocks / ((double)ms * 1e-3);
+  c->launches += 2;
+  return check(c);
+}
+
 // dense staging arrays for the *_host entry points live in the (dead between steps)
 // star-group slots S_ST.. (8 padded slots >= 6 dense arrays)
 template <class T> T* staging(cspt_ctx* c, int f) { return field<T>(c, S_ST + f); }
@@ -717,6 +741,13 @@ int cspt_run_cfl(cspt_ctx* c, double cfl, int nsteps, double* t_host_out) {
   if (!c->has_state) return CSPT_ESTATE;
   if (c->cuda_error) return CSPT_ECUDA;
   return DISPATCH(c, run_cfl_t)(c, cfl, nsteps, t_host_out);
+}
+
+int cspt_probe_fma_rate(cspt_ctx* c, int other_per_fma, double* fma_per_second) {
+  if (!c || !fma_per_second) return CSPT_EINVAL;
+  if (other_per_fma != 0 && other_per_fma != 2 && other_per_fma != 4 && other_per_fma != 8) return CSPT_EINVAL;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, probe_fma_t)(c, other_per_fma, fma_per_second);
 }
 
 int cspt_get_state(cspt_ctx* c, void* rho, void* u, void* v, void* w, void* p) {
