@@ -428,7 +428,7 @@ def run_cspt(args):
     s.run_cfl(w.cfl, 2)                  # graph capture outside the timed region
     barrier()
     fma_rate = s.probe_fma_rate()        # roofline denominator, measured on this box in this run
-    issue_probe = {str(k): s.probe_fma_rate(k) for k in (2, 4, 8)}
+    issue_probe = {str(k): s.probe_fma_rate(k) for k in (1, 2, 4, 8)}
     barrier()
 
     # ---- timed region: exactly K steps (cspt_run_cfl), device time from CUDA events on the launching stream,
@@ -523,8 +523,9 @@ def run_cspt(args):
                                       clocks.get("sm_max_mhz") or 1965),
                     "fma_per_second": fma_rate,
                     "fma_per_second_with_other_instructions": issue_probe,
-                    "issue_note": "FMA rate with 2 / 4 / 8 independent integer instructions per FMA: time ~ slots(FMA) + "
-                                  "others, slots(FMA) = 2 in fp64 and 1 in fp32 (DESIGN.md section 7)",
+                    "issue_note": "FMA rate with 1 / 2 / 4 / 8 independent integer instructions behind every FMA: cycles per "
+                                  "FMA and SMSP ~ max(pipe, 1.1 * (1 + others)), pipe = 2 in fp64 and 1 in fp32 "
+                                  "(DESIGN.md section 7, profiles/r2_issue_model.md)",
                     "algorithmic_flops_per_cell": ALGO_FLOPS[dom],
                     "algorithmic_instr_per_cell": ALGO_INSTR[dom], "kernel_ms": dom_ms, "share_of_step": share,
                     "hbm": hbm}

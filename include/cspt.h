@@ -146,9 +146,10 @@ int cspt_profile_read(cspt_ctx*, int kid, double* total_ms, long long* launches)
 /* Roofline probe: runs a kernel of independent FMAs in the ctx's precision on every SM and
  * writes the measured rate, thread-level FMAs per second, to *fma_per_second (the denominator of bench.py's "alu"
  * roofline, taken on the same box under the same clocks as the timed steps).  other_per_fma = 0: FMAs only;
- * 2, 4 or 8: that many independent integer instructions interleaved per FMA, which shows how the FMAs share the
- * issue slots with everything else (an FP64 FMA takes two slots).  Uses workspace that is
- * dead between steps: call it between steps only.  Syncs.  EINVAL: other_per_fma not one of 0, 2, 4, 8. */
+ * 1, 2, 4 or 8: that many independent integer instructions behind every FMA, which shows how the FMAs share the
+ * issue port with everything else (an FP64 FMA holds its pipe for two cycles, one other instruction issues in its
+ * shadow, every further one costs about one issue cycle: DESIGN.md section 7).  Uses workspace that is dead between
+ * steps: call it between steps only.  Syncs.  EINVAL: other_per_fma not one of 0, 1, 2, 4, 8. */
 int cspt_probe_fma_rate(cspt_ctx*, int other_per_fma, double* fma_per_second);
 /* The cudaError_t value behind a CSPT_ECUDA status of this ctx (0 if none). */
 int cspt_cuda_error(const cspt_ctx*);

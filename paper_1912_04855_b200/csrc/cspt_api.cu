@@ -298,7 +298,7 @@ bool corr_select(cspt_ctx* c, const Params<T>* P, const T* U) {
 template <class T, int TY, int MINB, int LIM, int RIEM>
 bool euler2_kernel(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
   typedef Euler2Smem<T, TY> S;
-  auto kern = k_euler_rows<T, TY, MINB, LIM, RIEM>;
+  auto kern = c->euler_variant == 5 ? k_euler_rows<T, TY, MINB, LIM, RIEM, 2> : k_euler_rows<T, TY, MINB, LIM, RIEM>;
   if (!P) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) == cudaSuccess;
   const Layout& L = c->L;
   int gx = (L.nx + S::TX - 1) / S::TX, gy = (L.ny + TY - 1) / TY;
@@ -360,6 +360,7 @@ bool euler_select(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
     case 2: return euler2_variant<T, 7, 2>(c, P, U, UN);
     case 3: return euler2_variant<T, 7, 3>(c, P, U, UN);
     case 4: return euler2_variant<T, 7, 4>(c, P, U, UN);
+    case 5: return euler2_variant<T, 7, 2>(c, P, U, UN);
     default: return false;
   }
 }
@@ -529,7 +530,11 @@ int probe_fma_t(cspt_ctx* c, int other_per_fma, double* fma_per_second) {
   T* out = field<T>(c, S_ST);
   const int threads = 128, blocks = 148 * 8, iters = other_per_fma ? 1500 : 4000;
   if ((long long)threads * blocks > c->L.fstride * 8) return CSPT_EINVAL;
-  auto kern = other_per_fma == 0 ? k_probe_fma<T, 0> : other_per_fma == 2 ? k_probe_fma<T, 1> : other_per_fma == 4 ? k_probe_fma<T, 2> : k_probe_fma<T, 4>;
+  auto kern = other_per_fma == 0   ? k_probe_fma<T, 0>
+              : other_per_fma == 1 ? k_probe_fma<T, 1>
+              : other_per_fma == 2 ? k_probe_fma<T, 2>
+              : other_per_fma == 4 ? k_probe_fma<T, 4>
+                                   : k_probe_fma<T, 8>;
   cudaEvent_t e0, e1;
   if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { (void)cudaGetLastError(); return CSPT_ECUDA; }
   kern<<<blocks, threads, 0, c->stream>>>(out, 200, (T)1.0000001, (T)1e-9, 5);          // warm-up
@@ -596,7 +601,7 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   // the issue slots of its FP64 instructions and runs the pair-symmetric corrector and the row-per-warp Euler
   // stage; fp32 keeps the packed-f32x2 corrector and the one-thread-per-cell Euler stage at 4 CTAs per SM
   c->corr_variant = dtype == CSPT_F64 ? 2 : 0;
-  c->euler_variant = dtype == CSPT_F64 ? 2 : 0;
+  c->euler_variant = dtype == CSPT_F64 ? 5 : 0;
   if (const char* e = getenv("CSPT_CORR")) c->corr_variant = atoi(e);        // development switches (A/B runs)
   if (const char* e = getenv("CSPT_EULER")) c->euler_variant = atoi(e);
   if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
@@ -712,7 +717,7 @@ int cspt_set_riemann(cspt_ctx* c, int riemann) {
   // the LF and HLLC fluxes need both states at a face: only the row layout of the Euler stage exchanges states, so a
   // ctx on the cell-per-thread layout (fp32 default) moves to the row layout (new tensor maps, host side only)
   if (riemann != CSPT_RIEMANN_HLL && c->euler_variant == 0) {
-    c->euler_variant = c->dtype == CSPT_F64 ? 2 : 3;
+    c->euler_variant = c->dtype == CSPT_F64 ? 5 : 3;
     bool ok = c->dtype == CSPT_F64 ? euler_select<double>(c, nullptr, nullptr, nullptr)
                                    : euler_select<float>(c, nullptr, nullptr, nullptr);
     if (!ok) { (void)cudaGetLastError(); c->cuda_error = (int)cudaErrorUnknown; return CSPT_ECUDA; }
@@ -745,7 +750,8 @@ int cspt_run_cfl(cspt_ctx* c, double cfl, int nsteps, double* t_host_out) {
 
 int cspt_probe_fma_rate(cspt_ctx* c, int other_per_fma, double* fma_per_second) {
   if (!c || !fma_per_second) return CSPT_EINVAL;
-  if (other_per_fma != 0 && other_per_fma != 2 && other_per_fma != 4 && other_per_fma != 8) return CSPT_EINVAL;
+  if (other_per_fma != 0 && other_per_fma != 1 && other_per_fma != 2 && other_per_fma != 4 && other_per_fma != 8)
+    return CSPT_EINVAL;
   if (c->cuda_error) return CSPT_ECUDA;
   return DISPATCH(c, probe_fma_t)(c, other_per_fma, fma_per_second);
 }

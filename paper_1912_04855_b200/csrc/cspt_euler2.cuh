@@ -1,8 +1,9 @@
 // cspt_euler2.cuh -- Eulerian stage, second layout: FGC (Eq. (8) + Riemann flux) and SUE (Eq. (4)), PAPER.md:45-50,
 // :70-78, :112-113; readings G9-G14, with the CFL signal speed of U^{n+1} (G15) as epilogue.
 //
-// What bounds this kernel on B200 is the instruction issue rate (an FP64 instruction takes two issue slots and nothing
-// issues beside it, profiles/r2_issue_model.md), so the layout minimises instructions per cell:
+// What bounds this kernel on B200 is the instruction issue rate (one instruction per cycle and SM sub-partition; only a
+// third of its instructions are FP64 arithmetic, profiles/r2_issue_model.md), so the layout minimises instructions per
+// cell; the z loop is unrolled twice (UNR) so that the registers carried from plane to plane are renamed, not moved:
 //   * one CTA = TY main warps (warp = one row of 32 cells, one cell per thread and plane) + ONE helper warp, streaming
 //     along z (2.5-D) over a 2-stage TMA ring of U^n (halo 2) and (U~, xi) (halo 1);
 //   * per cell and axis the two EDGE quantities are formed once:  P_i belongs to face i+1/2, M_i to face i-1/2, and the
@@ -110,7 +111,7 @@ struct Euler2Smem {
   static constexpr int THREADS = TX * (TY + 1);
 };
 
-template <class T, int TY, int MINB, int LIM, int RIEM>
+template <class T, int TY, int MINB, int LIM, int RIEM, int UNR = 1>
 __global__ void __launch_bounds__(32 * (TY + 1), MINB)
 k_euler_rows(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL, Params<T> P,
              const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, T* __restrict__ UN,
@@ -184,6 +185,7 @@ k_euler_rows(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ C
     for (int q = 0; q < 5; ++q) U0[q] = sU[(q * S::UY + (ty + 2)) * S::BX + (tx + S::HX)];
   }
 
+#pragma unroll UNR
   for (int p = z0 - 1; p <= z1; ++p) {
     const T* sU = (const T*)(sm + S::OFF_U + slotU(p) * S::U_STAGE);
     const T* sL = (const T*)(sm + S::OFF_L + slotL(p) * S::L_STAGE);

@@ -337,25 +337,32 @@ __global__ void k_reset_smax(DevScalars<T>* sc, int reset_time) {
 }
 
 // ---- roofline probe: the FMA rate of the plain FP64 / FP32 pipe, measured on the box the bench runs on ----------
-// Eight independent FMA chains per thread; NI > 0 adds 2 NI independent integer instructions per FMA (four chains of
-// xor + add) to show how other instructions share the issue slots with the FMAs (profiles/r2_issue_model.md).
+// Eight independent FMA chains per thread; NI > 0 puts NI independent integer instructions (add / xor on eight
+// chains of their own) behind every FMA, to show how other instructions share the issue port with the FMAs
+// (profiles/r2_issue_model.md: an FP64 FMA holds its pipe for two cycles but ONE other instruction issues in its
+// shadow; beyond that every instruction costs about 1.1 issue cycles).
 template <class T, int NI>
 __global__ void k_probe_fma(T* out, int iters, T a, T b, int m) {
-  T x0 = (T)threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
-  int i0 = threadIdx.x, i1 = i0 * 3, i2 = i0 * 5, i3 = i0 * 7;
+  T x[8];
+  int i[8];
+#pragma unroll
+  for (int c = 0; c < 8; ++c) { x[c] = (T)(threadIdx.x + c); i[c] = (int)threadIdx.x * (2 * c + 3); }
   for (int it = 0; it < iters; ++it) {
 #pragma unroll
     for (int u = 0; u < 8; ++u) {
-      x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
-      x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
 #pragma unroll
-      for (int q = 0; q < NI; ++q) {
-        i0 = (i0 ^ m) + i1; i1 = (i1 ^ m) + i2; i2 = (i2 ^ m) + i3; i3 = (i3 ^ m) + i0;
-        i0 = (i0 ^ m) + i1; i1 = (i1 ^ m) + i2; i2 = (i2 ^ m) + i3; i3 = (i3 ^ m) + i0;
+      for (int c = 0; c < 8; ++c) {
+        x[c] = fma(x[c], a, b);
+#pragma unroll
+        for (int q = 0; q < NI; ++q) i[c] = (q & 1) ? (i[c] ^ m) : (i[c] + m);
       }
     }
   }
-  out[blockIdx.x * blockDim.x + threadIdx.x] = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7)) + (T)((i0 + i1) + (i2 + i3));
+  int isum = 0;
+  T xsum = 0;
+#pragma unroll
+  for (int c = 0; c < 8; ++c) { isum += i[c]; xsum += x[c]; }
+  out[blockIdx.x * blockDim.x + threadIdx.x] = xsum + (T)isum;
 }
 
 template <class T>
