@@ -35,7 +35,12 @@ typedef struct cspt_ctx cspt_ctx; /* opaque */
 
 enum { CSPT_F64 = 0, CSPT_F32 = 1 };
 /* boundary kind per face, order xlo,xhi,ylo,yhi,zlo,zhi (reading G16) */
-enum { CSPT_BC_PERIODIC = 0, CSPT_BC_OUTFLOW = 1, CSPT_BC_INFLOW = 2 };
+enum { CSPT_BC_PERIODIC = 0, CSPT_BC_OUTFLOW = 1, CSPT_BC_INFLOW = 2,
+       /* z faces only: the face borders another z slab of the same grid (multi-GPU decomposition);
+        * its ghost planes are not filled by a boundary rule but written by cspt_halo_put */
+       CSPT_BC_EXTERNAL = 3 };
+/* what a z-slab halo message carries: the five conserved fields of the current state, or the potential psi */
+enum { CSPT_HALO_U = 0, CSPT_HALO_PSI = 1 };
 /* TVD slope limiter of Eq. (8): minmod is the default (reading G12) */
 enum { CSPT_LIMITER_MINMOD = 0, CSPT_LIMITER_VANLEER = 1 };
 /* approximate Riemann solver of the Euler stage: HLL is the default (readings G13, G13b, G13c) */
@@ -54,7 +59,7 @@ size_t cspt_workspace_bytes(int nx, int ny, int nz, int dtype);
  * (NULL = default stream).
  * EINVAL: null out/bc/workspace, n < 1, n < 4 on a non-periodic axis, h <= 0,
  * gamma <= 1, one face of an axis periodic and the other not, unknown dtype or
- * boundary kind, workspace too small or misaligned.  In CSPT_F32 mode h, gamma,
+ * boundary kind, CSPT_BC_EXTERNAL on an x or y face, workspace too small or misaligned.  In CSPT_F32 mode h, gamma,
  * cfl and dt are rounded to float once at the API. */
 int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, const int bc[6],
                 int dtype, void* workspace, size_t workspace_bytes, void* cuda_stream);
@@ -151,6 +156,33 @@ int cspt_profile_read(cspt_ctx*, int kid, double* total_ms, long long* launches)
  * shadow, every further one costs about one issue cycle: DESIGN.md section 7).  Uses workspace that is dead between
  * steps: call it between steps only.  Syncs.  EINVAL: other_per_fma not one of 0, 1, 2, 4, 8. */
 int cspt_probe_fma_rate(cspt_ctx*, int other_per_fma, double* fma_per_second);
+/* ---- z-slab decomposition over several GPUs ("the computational domain is divided between GPUs",
+ * :123).  One ctx per slab of nz_local planes; a z face that borders another slab has
+ * kind CSPT_BC_EXTERNAL.  The dependence of one step reaches 3 cells (reading G16), and every intermediate
+ * field is evaluated on the extended domain from the ghost layers of U^n, so ONE exchange of the 3 ghost planes of the 5
+ * conserved fields per face and step (plus psi once per cspt_set_state, and one scalar min-reduction of the time step)
+ * makes the slabs advance exactly as the undivided grid does.  Protocol per step, the transport between the two
+ * calls being the caller's (NCCL send/recv, a peer copy, ...):
+ *     cspt_fill_ghosts;  cspt_halo_get(face) -> neighbour's cspt_halo_put(opposite face);  dt = min over slabs of
+ *     cspt_compute_dt;  cspt_step_filled(dt)
+ * and after cspt_set_state (which on such a ctx pads psi and stops):  cspt_halo_get/put(CSPT_HALO_PSI);
+ * cspt_finish_state.  cspt_step, cspt_step_cfl and cspt_run_cfl return ESTATE on a ctx with an EXTERNAL face.
+ *
+ * cspt_halo_elems: elements of one halo message: (5 | 1) fields x 3 planes x the xy-PADDED plane (the x and y ghost
+ *   layers travel with the plane: the z fill of reading G16 runs over the xy-padded array).
+ * cspt_halo_get: copies the 3 interior planes next to z face `face` (4: z-lo, 5: z-hi), field by field, plane index
+ *   ascending, into the device buffer buf.  CSPT_HALO_U: call after cspt_fill_ghosts (x and y ghosts must be current);
+ *   CSPT_HALO_PSI: between cspt_set_state and cspt_finish_state.  EINVAL: face not 4 or 5, nz < 3.
+ * cspt_halo_put: writes such a message into the 3 ghost planes of `face`, which must be EXTERNAL (else EINVAL).
+ * cspt_finish_state: forms f = -D[psi] (S2) once the psi ghost planes are in place; ESTATE if no cspt_set_state is
+ *   pending.  cspt_fill_ghosts: S0 on every face that is not EXTERNAL.  cspt_step_filled: S1..S9 with the given dt on a
+ *   state whose ghost layers are complete.  All enqueue on the ctx's stream and do not sync. */
+int cspt_halo_elems(const cspt_ctx*, int what, long long* elems);
+int cspt_halo_get(cspt_ctx*, int face, int what, void* device_buf);
+int cspt_halo_put(cspt_ctx*, int face, int what, const void* device_buf);
+int cspt_finish_state(cspt_ctx*);
+int cspt_fill_ghosts(cspt_ctx*);
+int cspt_step_filled(cspt_ctx*, double dt);
 /* The cudaError_t value behind a CSPT_ECUDA status of this ctx (0 if none). */
 int cspt_cuda_error(const cspt_ctx*);
 /* Waits for the ctx's stream. */

@@ -10,7 +10,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcspt.so")
 
 F64, F32 = 0, 1
-BC_PERIODIC, BC_OUTFLOW, BC_INFLOW = 0, 1, 2
+BC_PERIODIC, BC_OUTFLOW, BC_INFLOW, BC_EXTERNAL = 0, 1, 2, 3
+HALO_U, HALO_PSI = 0, 1
 LIMITER_MINMOD, LIMITER_VANLEER = 0, 1
 KERNEL_CUBIC_SPLINE, KERNEL_POLY5 = 0, 1
 RIEMANN_HLL, RIEMANN_LF, RIEMANN_HLLC = 0, 1, 2
@@ -42,6 +43,12 @@ SYMBOLS = [
     ("cspt_profile_kernel_name", ctypes.c_char_p, [_ci]),
     ("cspt_profile_read", _ci, [_vp, _ci, _pd, ctypes.POINTER(ctypes.c_longlong)]),
     ("cspt_probe_fma_rate", _ci, [_vp, _ci, _pd]),
+    ("cspt_halo_elems", _ci, [_vp, _ci, ctypes.POINTER(ctypes.c_longlong)]),
+    ("cspt_halo_get", _ci, [_vp, _ci, _ci, _vp]),
+    ("cspt_halo_put", _ci, [_vp, _ci, _ci, _vp]),
+    ("cspt_finish_state", _ci, [_vp]),
+    ("cspt_fill_ghosts", _ci, [_vp]),
+    ("cspt_step_filled", _ci, [_vp, _cd]),
     ("cspt_cuda_error", _ci, [_vp]),
     ("cspt_sync", _ci, [_vp]),
     ("cspt_destroy", None, [_vp]),
@@ -244,6 +251,35 @@ class Solver:
         out = ctypes.c_double()
         _check(lib().cspt_probe_fma_rate(self._h, int(other_per_fma), ctypes.byref(out)), "cspt_probe_fma_rate")
         return out.value
+
+    # -- z-slab decomposition (include/cspt.h: CSPT_BC_EXTERNAL) ---------------------------------------
+    def halo_elems(self, what=HALO_U):
+        n = ctypes.c_longlong()
+        _check(lib().cspt_halo_elems(self._h, int(what), ctypes.byref(n)), "cspt_halo_elems")
+        return int(n.value)
+
+    def halo_get(self, face, what=HALO_U, out=None):
+        if out is None:
+            out = self.torch.empty(self.halo_elems(what), dtype=self.tdtype, device=self.device)
+        self._before()
+        _check(lib().cspt_halo_get(self._h, int(face), int(what), _dptr(out)), "cspt_halo_get")
+        self._after()
+        return out
+
+    def halo_put(self, face, buf, what=HALO_U):
+        assert buf.is_cuda and buf.dtype == self.tdtype and buf.is_contiguous() and buf.numel() == self.halo_elems(what)
+        self._before()
+        _check(lib().cspt_halo_put(self._h, int(face), int(what), _dptr(buf)), "cspt_halo_put")
+        self._after()
+
+    def finish_state(self):
+        _check(lib().cspt_finish_state(self._h), "cspt_finish_state")
+
+    def fill_ghosts(self):
+        _check(lib().cspt_fill_ghosts(self._h), "cspt_fill_ghosts")
+
+    def step_filled(self, dt):
+        _check(lib().cspt_step_filled(self._h, float(dt)), "cspt_step_filled")
 
     def cuda_error(self):
         return int(lib().cspt_cuda_error(self._h))

@@ -121,6 +121,50 @@ void fill_ghosts(cspt_ctx* c, T* F, int nfields, int mode) {
   }
 }
 
+inline bool has_external(const cspt_ctx* c) { return c->bc[4] == CSPT_BC_EXTERNAL || c->bc[5] == CSPT_BC_EXTERNAL; }
+
+// S2: f = -D[psi] on interior(+)2 from the padded psi (all ghost layers filled)
+template <class T>
+int finish_state_t(cspt_ctx* c) {
+  Params<T> P = make_params<T>(c);
+  T* psi_pad = field<T>(c, S_UT);          // scratch: U~ is dead between steps
+  long long ne = (long long)(c->L.nx + 4) * (c->L.ny + 4) * (c->L.nz + 4);
+  LAUNCH(c, K_FORCE, k_force<T>, blocks_for(ne, TPB, STRIDE_CAP), TPB, P, psi_pad, field<T>(c, S_F));
+  c->force_pending = false;
+  c->has_state = true;
+  return check(c);
+}
+
+// z-slab halo: NG xy-padded planes are contiguous in a padded field.  get: the interior
+// planes next to the face; put: the ghost planes of the face.
+template <class T>
+int halo_copy_t(cspt_ctx* c, int face, int what, void* buf, bool put) {
+  const Layout& L = c->L;
+  const long long plane = (long long)L.px * L.py, chunk = NG * plane;
+  const int nf = what == CSPT_HALO_U ? 5 : 1;
+  T* F = what == CSPT_HALO_U ? field<T>(c, c->cur ? S_U1 : S_U0) : field<T>(c, S_UT);
+  // first padded plane of the region: ghost planes [0, NG) | [NG + nz, 2 NG + nz), interior planes [NG, 2 NG) | [nz, nz + NG)
+  long long k0;
+  if (put) k0 = face == 4 ? 0 : NG + L.nz;
+  else k0 = face == 4 ? NG : L.nz;
+  int ps_ = prof_open(c, K_IO);
+  for (int f = 0; f < nf; ++f) {
+    T* fld = F + f * L.fstride + k0 * plane;
+    T* b = (T*)buf + f * chunk;
+    cudaError_t e = put ? cudaMemcpyAsync(fld, b, chunk * sizeof(T), cudaMemcpyDeviceToDevice, c->stream)
+                        : cudaMemcpyAsync(b, fld, chunk * sizeof(T), cudaMemcpyDeviceToDevice, c->stream);
+    if (e != cudaSuccess) { c->cuda_error = (int)e; return CSPT_ECUDA; }
+  }
+  prof_close(c, ps_);
+  return check(c);
+}
+
+template <class T>
+int fill_ghosts_t(cspt_ctx* c) {
+  fill_ghosts<T>(c, field<T>(c, c->cur ? S_U1 : S_U0), 5, 0);
+  return check(c);
+}
+
 template <class T>
 int set_state_t(cspt_ctx* c, const void* rho, const void* u, const void* v, const void* w, const void* p, const void* psi) {
   Params<T> P = make_params<T>(c);
@@ -130,14 +174,16 @@ int set_state_t(cspt_ctx* c, const void* rho, const void* u, const void* v, cons
   LAUNCH(c, K_IO, k_set_state<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, (const T*)rho, (const T*)u, (const T*)v,
          (const T*)w, (const T*)p, (const T*)psi, U, psi_pad);
   fill_ghosts<T>(c, psi_pad, 1, 2);
-  long long ne = (long long)(c->L.nx + 4) * (c->L.ny + 4) * (c->L.nz + 4);
-  LAUNCH(c, K_FORCE, k_force<T>, blocks_for(ne, TPB, STRIDE_CAP), TPB, P, psi_pad, field<T>(c, S_F));
   fill_ghosts<T>(c, U, 5, 1);
   LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, scalars<T>(c), 1);
   c->cur = 0;
-  c->has_state = true;
   c->smax_valid = false;
-  return check(c);
+  c->has_state = false;
+  c->force_pending = true;
+  // a slab (EXTERNAL z faces) needs the psi ghost planes of its neighbours before f = -D[psi] can be formed there:
+  // cspt_halo_get/put(CSPT_HALO_PSI), then cspt_finish_state
+  if (has_external(c)) return check(c);
+  return finish_state_t<T>(c);
 }
 
 template <class T>
@@ -285,20 +331,16 @@ bool pair_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
 template <class T>
 bool corr_select(cspt_ctx* c, const Params<T>* P, const T* U) {
   const bool xp = c->bc[0] == CSPT_BC_PERIODIC;
-  switch (c->corr_variant) {
-    case 1: return xp ? pair_variant<T, 8, 4, 2, 1, 0>(c, P, U) : pair_variant<T, 8, 4, 2, 0, 0>(c, P, U);
-    case 2: return xp ? pair_variant<T, 8, 4, 2, 1, 1>(c, P, U) : pair_variant<T, 8, 4, 2, 0, 1>(c, P, U);
-    case 3: return xp ? pair_variant<T, 8, 3, 3, 1, 1>(c, P, U) : pair_variant<T, 8, 3, 3, 0, 1>(c, P, U);
-    default: return corr_dispatch<T>(c, P, U);
-  }
+  if (c->corr_variant == 0) return corr_dispatch<T>(c, P, U);
+  return xp ? pair_variant<T, 8, 4, 2, 1, 1>(c, P, U) : pair_variant<T, 8, 4, 2, 0, 1>(c, P, U);
 }
 
 // Euler stage, second layout (cspt_euler2.cuh): TY rows of 32 cells + one helper warp per CTA.
 // P == nullptr: tensor maps and dynamic shared memory; otherwise launch.
-template <class T, int TY, int MINB, int LIM, int RIEM>
+template <class T, int TY, int MINB, int UNR, int LIM, int RIEM>
 bool euler2_kernel(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
   typedef Euler2Smem<T, TY> S;
-  auto kern = c->euler_variant == 5 ? k_euler_rows<T, TY, MINB, LIM, RIEM, 2> : k_euler_rows<T, TY, MINB, LIM, RIEM>;
+  auto kern = k_euler_rows<T, TY, MINB, LIM, RIEM, UNR>;
   if (!P) return cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) == cudaSuccess;
   const Layout& L = c->L;
   int gx = (L.nx + S::TX - 1) / S::TX, gy = (L.ny + TY - 1) / TY;
@@ -312,7 +354,7 @@ bool euler2_kernel(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
   return true;
 }
 
-template <class T, int TY, int MINB>
+template <class T, int TY, int MINB, int UNR>
 bool euler2_variant(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
   typedef Euler2Smem<T, TY> S;
   const Layout& L = c->L;
@@ -322,15 +364,15 @@ bool euler2_variant(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
       ok = ok && make_field_map(&c->mapU[b], field<T>(c, b ? S_U1 : S_U0), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 5,
                                 S::BX, S::UY, 5);
     ok = ok && make_field_map(&c->mapL, field<T>(c, S_UT), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 7, S::BX, S::LY, 7);
-    return ok && euler2_kernel<T, TY, MINB, 0, 0>(c, P, U, UN) && euler2_kernel<T, TY, MINB, 1, 0>(c, P, U, UN) &&
-           euler2_kernel<T, TY, MINB, 0, 1>(c, P, U, UN) && euler2_kernel<T, TY, MINB, 1, 1>(c, P, U, UN) &&
-           euler2_kernel<T, TY, MINB, 0, 2>(c, P, U, UN) && euler2_kernel<T, TY, MINB, 1, 2>(c, P, U, UN);
+    return ok && euler2_kernel<T, TY, MINB, UNR, 0, 0>(c, P, U, UN) && euler2_kernel<T, TY, MINB, UNR, 1, 0>(c, P, U, UN) &&
+           euler2_kernel<T, TY, MINB, UNR, 0, 1>(c, P, U, UN) && euler2_kernel<T, TY, MINB, UNR, 1, 1>(c, P, U, UN) &&
+           euler2_kernel<T, TY, MINB, UNR, 0, 2>(c, P, U, UN) && euler2_kernel<T, TY, MINB, UNR, 1, 2>(c, P, U, UN);
   }
   const bool vl = c->limiter == CSPT_LIMITER_VANLEER;
   switch (c->riemann) {
-    case CSPT_RIEMANN_LF: return vl ? euler2_kernel<T, TY, MINB, 1, 1>(c, P, U, UN) : euler2_kernel<T, TY, MINB, 0, 1>(c, P, U, UN);
-    case CSPT_RIEMANN_HLLC: return vl ? euler2_kernel<T, TY, MINB, 1, 2>(c, P, U, UN) : euler2_kernel<T, TY, MINB, 0, 2>(c, P, U, UN);
-    default: return vl ? euler2_kernel<T, TY, MINB, 1, 0>(c, P, U, UN) : euler2_kernel<T, TY, MINB, 0, 0>(c, P, U, UN);
+    case CSPT_RIEMANN_LF: return vl ? euler2_kernel<T, TY, MINB, UNR, 1, 1>(c, P, U, UN) : euler2_kernel<T, TY, MINB, UNR, 0, 1>(c, P, U, UN);
+    case CSPT_RIEMANN_HLLC: return vl ? euler2_kernel<T, TY, MINB, UNR, 1, 2>(c, P, U, UN) : euler2_kernel<T, TY, MINB, UNR, 0, 2>(c, P, U, UN);
+    default: return vl ? euler2_kernel<T, TY, MINB, UNR, 1, 0>(c, P, U, UN) : euler2_kernel<T, TY, MINB, UNR, 0, 0>(c, P, U, UN);
   }
 }
 
@@ -353,16 +395,13 @@ bool euler1_setup(cspt_ctx* c) {
   return ok;
 }
 
+// Row layout: 7 rows + helper warp per CTA; fp64 at 2 CTAs per SM (128 registers) with the z loop unrolled twice,
+// fp32 at 3 CTAs per SM (the fastest of the shapes measured, profiles/r2_kernels.md)
 template <class T>
 bool euler_select(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
-  switch (c->euler_variant) {
-    case 1: return euler2_variant<T, 8, 2>(c, P, U, UN);
-    case 2: return euler2_variant<T, 7, 2>(c, P, U, UN);
-    case 3: return euler2_variant<T, 7, 3>(c, P, U, UN);
-    case 4: return euler2_variant<T, 7, 4>(c, P, U, UN);
-    case 5: return euler2_variant<T, 7, 2>(c, P, U, UN);
-    default: return false;
-  }
+  if (c->euler_variant == 0) return false;
+  if constexpr (sizeof(T) == 8) return euler2_variant<T, 7, 2, 2>(c, P, U, UN);
+  else return euler2_variant<T, 7, 3, 1>(c, P, U, UN);
 }
 
 template <class T>
@@ -413,12 +452,11 @@ void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
 }
 
 template <class T>
-void run_step(cspt_ctx* c) {
+void run_step(cspt_ctx* c, bool fill = true) {
   Params<T> P = make_params<T>(c);
-  const Layout& L = c->L;
   T* U = field<T>(c, c->cur ? S_U1 : S_U0);
   T* UN = field<T>(c, c->cur ? S_U0 : S_U1);
-  fill_ghosts<T>(c, U, 5, 0);                                                      // O0
+  if (fill) fill_ghosts<T>(c, U, 5, 0);                                            // O0
   launch_predictor<T>(c, P, U);                                                    // O1, O3, O4
   launch_corrector<T>(c, P, U);                                                    // O5, O6
   launch_euler<T>(c, P, U, UN);                                                  // O7, O8 (+O9 epilogue)
@@ -430,6 +468,13 @@ template <class T>
 int step_t(cspt_ctx* c, double dt) {
   LAUNCH(c, K_SCALAR, k_set_dt<T>, 1, 1, scalars<T>(c), (T)dt);
   run_step<T>(c);
+  return check(c);
+}
+
+template <class T>
+int step_filled_t(cspt_ctx* c, double dt) {
+  LAUNCH(c, K_SCALAR, k_set_dt<T>, 1, 1, scalars<T>(c), (T)dt);
+  run_step<T>(c, false);
   return check(c);
 }
 
@@ -580,7 +625,8 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   int n[3] = {nx, ny, nz};
   for (int d = 0; d < 3; ++d) {
     int lo = bc[2 * d], hi = bc[2 * d + 1];
-    if (lo < 0 || lo > 2 || hi < 0 || hi > 2) return CSPT_EINVAL;
+    const int kmax = d == 2 ? CSPT_BC_EXTERNAL : CSPT_BC_INFLOW;         // EXTERNAL: z faces only (slab decomposition)
+    if (lo < 0 || lo > kmax || hi < 0 || hi > kmax) return CSPT_EINVAL;
     if ((lo == CSPT_BC_PERIODIC) != (hi == CSPT_BC_PERIODIC)) return CSPT_EINVAL;
     if (lo != CSPT_BC_PERIODIC && n[d] < 4) return CSPT_EINVAL;
   }
@@ -600,8 +646,8 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   // kernel layouts per precision, each the fastest measured on B200 (profiles/r2_kernels.md): fp64 is bound by
   // the issue slots of its FP64 instructions and runs the pair-symmetric corrector and the row-per-warp Euler
   // stage; fp32 keeps the packed-f32x2 corrector and the one-thread-per-cell Euler stage at 4 CTAs per SM
-  c->corr_variant = dtype == CSPT_F64 ? 2 : 0;
-  c->euler_variant = dtype == CSPT_F64 ? 5 : 0;
+  c->corr_variant = dtype == CSPT_F64 ? 1 : 0;
+  c->euler_variant = dtype == CSPT_F64 ? 1 : 0;
   if (const char* e = getenv("CSPT_CORR")) c->corr_variant = atoi(e);        // development switches (A/B runs)
   if (const char* e = getenv("CSPT_EULER")) c->euler_variant = atoi(e);
   if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
@@ -717,7 +763,7 @@ int cspt_set_riemann(cspt_ctx* c, int riemann) {
   // the LF and HLLC fluxes need both states at a face: only the row layout of the Euler stage exchanges states, so a
   // ctx on the cell-per-thread layout (fp32 default) moves to the row layout (new tensor maps, host side only)
   if (riemann != CSPT_RIEMANN_HLL && c->euler_variant == 0) {
-    c->euler_variant = c->dtype == CSPT_F64 ? 5 : 3;
+    c->euler_variant = 1;
     bool ok = c->dtype == CSPT_F64 ? euler_select<double>(c, nullptr, nullptr, nullptr)
                                    : euler_select<float>(c, nullptr, nullptr, nullptr);
     if (!ok) { (void)cudaGetLastError(); c->cuda_error = (int)cudaErrorUnknown; return CSPT_ECUDA; }
@@ -729,23 +775,68 @@ int cspt_set_riemann(cspt_ctx* c, int riemann) {
 
 int cspt_step(cspt_ctx* c, double dt) {
   if (!c || !(dt > 0) || !isfinite(dt)) return CSPT_EINVAL;
-  if (!c->has_state) return CSPT_ESTATE;
+  if (!c->has_state || has_external(c)) return CSPT_ESTATE;
   if (c->cuda_error) return CSPT_ECUDA;
   return DISPATCH(c, step_t)(c, dt);
 }
 
 int cspt_step_cfl(cspt_ctx* c, double cfl, double* dt_host_out) {
   if (!c || !(cfl > 0) || !isfinite(cfl)) return CSPT_EINVAL;
-  if (!c->has_state) return CSPT_ESTATE;
+  if (!c->has_state || has_external(c)) return CSPT_ESTATE;
   if (c->cuda_error) return CSPT_ECUDA;
   return DISPATCH(c, step_cfl_t)(c, cfl, dt_host_out);
 }
 
 int cspt_run_cfl(cspt_ctx* c, double cfl, int nsteps, double* t_host_out) {
   if (!c || !(cfl > 0) || !isfinite(cfl) || nsteps < 0) return CSPT_EINVAL;
-  if (!c->has_state) return CSPT_ESTATE;
+  if (!c->has_state || has_external(c)) return CSPT_ESTATE;
   if (c->cuda_error) return CSPT_ECUDA;
   return DISPATCH(c, run_cfl_t)(c, cfl, nsteps, t_host_out);
+}
+
+// ---- z-slab decomposition ------------------------------------------
+int cspt_halo_elems(const cspt_ctx* c, int what, long long* elems) {
+  if (!c || !elems || (what != CSPT_HALO_U && what != CSPT_HALO_PSI)) return CSPT_EINVAL;
+  *elems = (long long)(what == CSPT_HALO_U ? 5 : 1) * NG * c->L.px * c->L.py;
+  return CSPT_OK;
+}
+
+int cspt_halo_get(cspt_ctx* c, int face, int what, void* buf) {
+  if (!c || !buf || (face != 4 && face != 5) || (what != CSPT_HALO_U && what != CSPT_HALO_PSI)) return CSPT_EINVAL;
+  if (c->L.nz < NG) return CSPT_EINVAL;
+  if (what == CSPT_HALO_U ? !c->has_state : !c->force_pending) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return c->dtype == CSPT_F64 ? halo_copy_t<double>(c, face, what, buf, false) : halo_copy_t<float>(c, face, what, buf, false);
+}
+
+int cspt_halo_put(cspt_ctx* c, int face, int what, const void* buf) {
+  if (!c || !buf || (face != 4 && face != 5) || (what != CSPT_HALO_U && what != CSPT_HALO_PSI)) return CSPT_EINVAL;
+  if (c->bc[face] != CSPT_BC_EXTERNAL) return CSPT_EINVAL;
+  if (what == CSPT_HALO_U ? !c->has_state : !c->force_pending) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return c->dtype == CSPT_F64 ? halo_copy_t<double>(c, face, what, (void*)buf, true)
+                              : halo_copy_t<float>(c, face, what, (void*)buf, true);
+}
+
+int cspt_finish_state(cspt_ctx* c) {
+  if (!c) return CSPT_EINVAL;
+  if (!c->force_pending) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, finish_state_t)(c);
+}
+
+int cspt_fill_ghosts(cspt_ctx* c) {
+  if (!c) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, fill_ghosts_t)(c);
+}
+
+int cspt_step_filled(cspt_ctx* c, double dt) {
+  if (!c || !(dt > 0) || !isfinite(dt)) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, step_filled_t)(c, dt);
 }
 
 int cspt_probe_fma_rate(cspt_ctx* c, int other_per_fma, double* fma_per_second) {

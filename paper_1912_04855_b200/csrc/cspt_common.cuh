@@ -101,6 +101,7 @@ struct cspt_ctx {
   cudaStream_t stream;
   int cur;                 // which U buffer holds U^n
   bool has_state;
+  bool force_pending;      // cspt_set_state on a slab: psi is padded, f = -D[psi] waits for cspt_finish_state
   bool smax_valid;         // smax_bits on the device belongs to the current U^n
   int cuda_error;          // sticky
   long long launches;
@@ -115,8 +116,8 @@ struct cspt_ctx {
   int kernel;               // CSPT_KERNEL_*: smoothing kernel W of Eq. (7)
   int limiter;              // CSPT_LIMITER_*: TVD slope of Eq. (8) in the Euler stage
   int riemann;              // CSPT_RIEMANN_*: flux at the faces of the Euler stage
-  int euler_variant;        // 0: one thread per cell with shared-memory flux exchange, 1/2: rows + helper warp (TY = 8 / 7)
-  int corr_variant;         // 0: 26-neighbour corrector, 1: pair-symmetric strips, 2: + shared x pairs (warp shuffles)
+  int euler_variant;        // 0: one thread per cell with shared-memory flux exchange, 1: rows + helper warp
+  int corr_variant;         // 0: 26-neighbour corrector, 1: pair-symmetric strips with shared x pairs (warp shuffles)
   // CUDA graphs of two consecutive cspt_step_cfl steps (cspt_run_cfl), one per parity of `cur` at entry
   cudaGraphExec_t graph[2];
   cudaStream_t gstream;             // capture / replay stream of a ctx that lives on the legacy default stream

@@ -173,6 +173,7 @@ __global__ void k_ghost_axis(Layout L, int d, int mode, int bc_lo, int bc_hi, in
     else if (d == 1) { a = (int)(r % e2) + lo2; r /= e2; g = (int)(r % NG) + 1; r /= NG; side = (int)(r % 2); r /= 2; b = (int)r + lo1; }
     else { b = (int)(r % e1) + lo1; r /= e1; a = (int)(r % e2) + lo2; r /= e2; g = (int)(r % NG) + 1; side = (int)(r / NG); }
     int kind = side ? bc_hi : bc_lo;
+    if (kind == CSPT_BC_EXTERNAL) continue;            // ghost planes of a slab face: written by cspt_halo_put
     int q[3], s[3], e0[3];
     q[d1] = b; q[d2] = a; s[d1] = b; s[d2] = a; e0[d1] = b; e0[d2] = a;
     q[d] = side ? n[d] - 1 + g : -g;
