@@ -57,6 +57,9 @@ def parse():
                     help="smoothing kernel W of Eq. (7) (default: the reading the metric is quoted on)")
     ap.add_argument("--riemann", default="hll", choices=["hll", "lf", "hllc"],
                     help="Riemann solver of the Euler stage (default: the reading the metric is quoted on)")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent replicas (default; north_star has no domain decomposition) or ONE grid cut "
+                         "into z slabs over the ranks (SURVEY 8(f) NEXT-2, strong scaling)")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config throughput table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -567,10 +570,82 @@ def run_cspt(args):
         dist.destroy_process_group()
 
 
+def run_slab(args):
+    """ONE grid cut into z slabs over the ranks (paper_1912_04855_b200/slab.py): per step one halo exchange of 3 planes
+    x 5 fields per face over NCCL and one scalar min all-reduce.  Strong scaling: value = the grid's cells x steps / time."""
+    import torch
+    import torch.distributed as dist
+    from paper_1912_04855_b200 import build, cspt, slab
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the CSPH-TVD path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    if rank == 0:
+        build.build()
+    if world > 1:
+        dist.barrier()
+    cspt.lib()
+    w = make_workload(args)
+    dtype = cspt.F64 if w.dtype == "f64" else cspt.F32
+    s = slab.SlabSolver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, dtype, rank, world)
+    f = w.fields_slab(s.z0, s.z1)
+    s.set_state(*[torch.from_numpy(a.astype(w.np_dtype)).cuda() for a in f])
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        s.step_cfl(w.cfl)
+    barrier()
+    sampler = ClockSampler(local)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = s.solver.launch_count()
+    sampler.start()
+    e0.record(s.solver.stream)
+    for _ in range(args.steps):
+        s.step_cfl(w.cfl)
+    e1.record(s.solver.stream)
+    barrier()
+    clocks = sampler.stop()
+    tmax = max_over_ranks(e0.elapsed_time(e1), world, "cuda")
+    launches = s.solver.launch_count() - l0
+    rho = s.get_conserved()[0]
+    assert bool(torch.isfinite(rho).all()), "state is not finite after the timed steps"
+    halo = 2 * s.solver.halo_elems(cspt.HALO_U) * (8 if w.dtype == "f64" else 4)
+    s.close()
+    if rank == 0:
+        peak, _ = peaks()
+        esz = 8 if w.dtype == "f64" else 4
+        value = w.cells * args.steps / (tmax * 1e-3) / 1e6
+        ach = MIN_WORDS_PER_CELL * esz * w.cells / (tmax / args.steps * 1e-3) / 1e9
+        cfg = config_of(w, world)
+        cfg["parallelism"] = "z slabs over %d gpu(s): %d planes each, %d halo bytes per rank and step, one min all-reduce" % (
+            world, w.nz // world, halo)
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": tmax / args.steps, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": w.dtype, "data": "synthetic", "config": dict(cfg, api="slab.SlabSolver.step_cfl"),
+            "clocks": clocks, "gpu_launches": launches,
+            "step_hbm": {"bytes_per_cell_update": MIN_WORDS_PER_CELL * esz, "achieved_gbs": ach,
+                         "frac_of_measured_all_gpus": ach / (peak * world)}}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         run_reference(args)
+    elif args.decomp == "slab":
+        run_slab(args)
     else:
         run_cspt(args)
 
