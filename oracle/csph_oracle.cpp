@@ -18,11 +18,15 @@
 // uniform flow; Gamma=2 discrete hydrostatic equilibrium; conservation;
 // axis permutation / mirror; advected-sine convergence; vacuum fan closed
 // form; brute-force all-pairs evaluation of Eq. (7); closed-form lattice
-// weights; free fall in a linear potential.  Parity that stays UNPINNED:
-// agreement with the authors' own code (kernel, limiter, Riemann solver, CFL
-// rule and boundary rules are readings), the paper's
-// simple-wave order 1.94/2.04 (reading G23) and the Fig. 1
-// shock position (parameters missing from the paper).
+// weights; free fall in a linear potential; the ghost rules of every boundary
+// kind on non-uniform states, the pressure floor, the LF / HLL / HLLC face
+// fluxes against the textbook solvers; the paper's printed order 1.94 for the
+// linear transfer of a smooth wave on N = 400, 800, 1600 (reading
+// G23 (i)).  Parity that stays UNPINNED: agreement with the authors' own code
+// (kernel, limiter, Riemann solver, CFL rule and boundary rules are readings,
+// DESIGN.md section 3), second order on a nonlinear simple wave (reading
+// G23 (ii): measured first order) and the Fig. 1 shock position (parameters
+// missing from the paper).
 //
 // Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.sh).
 // -ffp-contract=off matters: the CFL time step and the vacuum mask are

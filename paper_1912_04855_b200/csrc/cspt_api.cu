@@ -294,7 +294,7 @@ bool corr_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
 }
 
 // 32 x 8 cells per plane, 2 cells per thread, 4 ring stages, 2 CTAs per SM (224 registers in fp64): the fastest of
-// the tile shapes tried on B200 in both precisions (profiles/r1h.md)
+// the tile shapes tried on B200 in round 1; the fp32 default (fp64 runs the pair-symmetric kernel below)
 template <class T>
 bool corr_dispatch(cspt_ctx* c, const Params<T>* P, const T* U) {
   return c->bc[0] == CSPT_BC_PERIODIC ? corr_variant<T, 32, 8, 2, 4, 2, 1>(c, P, U)
@@ -644,8 +644,8 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->stream = (cudaStream_t)cuda_stream;
   carve(c);
   // kernel layouts per precision, each the fastest measured on B200 (profiles/r2_kernels.md): fp64 is bound by
-  // the issue slots of its FP64 instructions and runs the pair-symmetric corrector and the row-per-warp Euler
-  // stage; fp32 keeps the packed-f32x2 corrector and the one-thread-per-cell Euler stage at 4 CTAs per SM
+  // the FP64 pipe and the issue port (profiles/r2_issue_model.md) and runs the pair-symmetric corrector and the
+  // row-per-warp Euler stage; fp32 keeps the packed-f32x2 corrector and the one-thread-per-cell Euler stage
   c->corr_variant = dtype == CSPT_F64 ? 1 : 0;
   c->euler_variant = dtype == CSPT_F64 ? 1 : 0;
   if (const char* e = getenv("CSPT_CORR")) c->corr_variant = atoi(e);        // development switches (A/B runs)

@@ -10,18 +10,19 @@
 // shared memory (the parts of the halo columns / rows are computed by the first / the last warps);
 // along z the thread keeps FP of the previous plane in registers and finishes cell p-1 when FM of
 // plane p is known.  The z+ neighbour U^n(p+1) of the own column is read from the other ring stage.
-// (A second layout with one warp per row, two halo-row warps and x exchange by warp shuffles was
-// measured slower in both precisions and removed: 6.1 / 4.2 ms against 5.4 / 3.3 ms at 512^3.)
+// This layout is the fp32 default for the HLL flux (4 CTAs of 64 registers per SM); fp64, and the LF / HLLC fluxes in
+// both precisions, run the row layout of cspt_euler2.cuh (profiles/r2_kernels.md has the A/B numbers).
 #pragma once
 #include "cspt_kernels.cuh"
 #include "cspt_tma.cuh"
 
 namespace cspt {
 
+// minmod(a, b) is the median of {a, b, 0}: four FMNMX in fp32 instead of two compares, two selects and a product
+// (where a or b is zero, or the signs differ, the median is that zero)
 template <class T>
 __device__ __forceinline__ T minmod_fast(T a, T b) {
-  T r = fabs(a) < fabs(b) ? a : b;
-  return a * b > (T)0 ? r : (T)0;
+  return fmaxf(fminf(a, b), fminf(fmaxf(a, b), 0.f));
 }
 // fp64: the sign agreement is tested on the high words (integer pipe instead of a DMUL and a DSETP on the FP64
 // pipe); where a or b is zero the smaller magnitude r is that zero, so the result is the same
