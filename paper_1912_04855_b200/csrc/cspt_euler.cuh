@@ -119,7 +119,7 @@ template <class T, int TX, int TY, int LIM>
 __global__ void __launch_bounds__(TX* TY, (sizeof(T) == 4 ? 1024 : 512) / (TX * TY))
 k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL, Params<T> P,
                const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, T* __restrict__ UN,
-               typename Real<T>::bits_t* __restrict__ smax_out, int zchunk) {
+               typename Real<T>::bits_t* __restrict__ smax_out, int* __restrict__ vac_next, int zchunk) {
   typedef EulerSmem<T, TX, TY> S;
   extern __shared__ __align__(128) unsigned char sm[];
   uint64_t* bar = (uint64_t*)(sm + S::OFF_BAR);
@@ -135,6 +135,7 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
   constexpr uint32_t TX_BYTES = (uint32_t)((S::U_ELEMS + S::L_ELEMS) * sizeof(T));
 
   if (tid == 0) {
+    *(int*)(bar + 4) = 0;
     mbar_init(&bar[0], 1);
     mbar_init(&bar[1], 1);
     mbar_fence_init();
@@ -154,6 +155,8 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
 
   const T dt = load_dt(sc);
   const T lam = dt * P.inv_h;
+  const bool vac_hint = sc->vac_cur != 0;          // U^n may hold vacuum cells: look for all-vacuum stencils
+  int* vac_seen = (int*)(bar + 4);                 // ... and does the U^{n+1} written here (flag in shared memory)
   T Um[5], FPzp[5], acc[5], Utp[5];
   // running maximum of the exact speeds seen by this thread, seeded with the global maximum so far (other
   // CTAs' exact speeds: a lower bound of the final maximum)
@@ -217,12 +220,22 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
           }
                 }
       };
+      // Gas-vacuum handling (G9): where the cell and its two neighbours along an axis all have rho <= rho_vac, the
+      // reconstructed densities lie between theirs, both face velocities are 0 and both flux parts vanish: a warp
+      // whose whole in-plane stencil is vacuum skips the reconstruction (most of the 1024^3 disk volume).
+      bool vac_xy = false;
+      if (vac_hint) {
+        const T rxy = fmax(fmax(fmax(u_at(0, ty, tx - 1), u_at(0, ty, tx + 1)), fmax(u_at(0, ty - 1, tx), u_at(0, ty + 1, tx))), U0[0]);
+        vac_xy = __all_sync(0xffffffffu, !(rxy > P.rho_vac));
+      }
       // ---- x axis -------------------------------------------------------------
       {
-        T Ux0[5], Ux1[5], FP[5], FM[5];
+        T Ux0[5], Ux1[5], FP[5] = {0, 0, 0, 0, 0}, FM[5] = {0, 0, 0, 0, 0};
+        if (!vac_xy) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) { Ux0[q] = u_at(q, ty, tx - 1); Ux1[q] = u_at(q, ty, tx + 1); }
-        flux_parts<T, 3, LIM>(P, 0, U0, Ux0, Ux1, hf, l_at(4, ty, tx), FP, FM);
+          for (int q = 0; q < 5; ++q) { Ux0[q] = u_at(q, ty, tx - 1); Ux1[q] = u_at(q, ty, tx + 1); }
+          flux_parts<T, 3, LIM>(P, 0, U0, Ux0, Ux1, hf, l_at(4, ty, tx), FP, FM);
+        }
         // exchange layout: [q][ty][tx+1], FP in 0..4, FM in 5..9, row pitch TX+2
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
@@ -258,10 +271,12 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
       }
       // ---- y axis -------------------------------------------------------------
       {
-        T Uy0[5], Uy1[5], FP[5], FM[5];
+        T Uy0[5], Uy1[5], FP[5] = {0, 0, 0, 0, 0}, FM[5] = {0, 0, 0, 0, 0};
+        if (!vac_xy) {
 #pragma unroll
-        for (int q = 0; q < 5; ++q) { Uy0[q] = u_at(q, ty - 1, tx); Uy1[q] = u_at(q, ty + 1, tx); }
-        flux_parts<T, 3, LIM>(P, 1, U0, Uy0, Uy1, hf, l_at(5, ty, tx), FP, FM);
+          for (int q = 0; q < 5; ++q) { Uy0[q] = u_at(q, ty - 1, tx); Uy1[q] = u_at(q, ty + 1, tx); }
+          flux_parts<T, 3, LIM>(P, 1, U0, Uy0, Uy1, hf, l_at(5, ty, tx), FP, FM);
+        }
         // exchange layout: [q][ty+1][tx], rows -1..TY, row pitch TX
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
@@ -286,7 +301,12 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
 #pragma unroll
       for (int q = 0; q < 5; ++q) Up[q] = sU1[(q * S::UY + (ty + 2)) * S::BX + (tx + S::HX)];
     }
-    flux_parts<T, 3, LIM>(P, 2, U0, Um, Up, hf, l_at(6, ty, tx), FPz, FMz);
+    if (vac_hint && __all_sync(0xffffffffu, !(fmax(fmax(Um[0], Up[0]), U0[0]) > P.rho_vac))) {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) FPz[q] = FMz[q] = (T)0;         // vacuum along z as well
+    } else {
+      flux_parts<T, 3, LIM>(P, 2, U0, Um, Up, hf, l_at(6, ty, tx), FPz, FMz);
+    }
     // finish cell p-1 (SUE, Eq. (4))
     if (p - 1 >= z0) {
       T un[5];
@@ -296,6 +316,7 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
         long long c = L.idx(i, j, p - 1);
 #pragma unroll
         for (int q = 0; q < 5; ++q) UN[c + q * fs] = un[q];
+        if (!(un[0] > P.rho_vac)) *vac_seen = 1;
         // CFL speed of U^{n+1} (G15): exactly rounded, but only for cells whose estimate comes within the
         // filter margin of a speed already known exactly (this thread's maximum or the global one so far);
         // the true maximum always passes the filter, so the result is the exact maximum
@@ -320,6 +341,8 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
     if (tid == 0 && p + 2 <= z1 + 1) issue(p + 2, s);
   }
   block_max_to_global<T>(smax, smax_out);
+  __syncthreads();
+  if (tid == 0 && *vac_seen) atomicOr(vac_next, 1);
 }
 
 }  // namespace cspt

@@ -375,9 +375,13 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
       for (int d = 0; d < 3; ++d) { ei[c][d][0] = ee[d] + (T)1; ei[c][d][1] = ee[d]; ei[c][d][2] = ee[d] - (T)1; }
       sx[c] = sy[c] = sz[c] = se[c] = (T)0;
     }
+    // a particle with phi = 0 (vacuum, or p floored to 0) neither exerts nor feels the pressure force: all four
+    // sums of such a cell are multiplied by phi_i = 0 in Eq. (7), so a warp whose own particles all have phi = 0
+    // skips the neighbour loop (gas-vacuum workloads: most of the 1024^3 disk volume)
     bool any = false;
 #pragma unroll
-    for (int c = 0; c < CY; ++c) any = any || valid[c];
+    for (int c = 0; c < CY; ++c) any = any || (valid[c] && phi_i[c] != (T)0);
+    any = __any_sync(0xffffffffu, any);
     // own-cell operands of Eq. (6) straight from global memory, requested before the neighbour loop
     // so that their latency is hidden behind it
     T own[CY][8];
