@@ -175,7 +175,7 @@ int set_state_t(cspt_ctx* c, const void* rho, const void* u, const void* v, cons
          (const T*)w, (const T*)p, (const T*)psi, U, psi_pad);
   fill_ghosts<T>(c, psi_pad, 1, 2);
   fill_ghosts<T>(c, U, 5, 1);
-  LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, scalars<T>(c), 3);
+  LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, scalars<T>(c), 1);
   c->cur = 0;
   c->smax_valid = false;
   c->has_state = false;
@@ -192,7 +192,6 @@ int set_conserved_t(cspt_ctx* c, const void* const in[5]) {
   T* U = field<T>(c, c->cur ? S_U1 : S_U0);
   for (int f = 0; f < 5; ++f)
     LAUNCH(c, K_IO, k_put_field<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, c->L, (const T*)in[f], U + f * c->L.fstride);
-  LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, scalars<T>(c), 2);
   c->smax_valid = false;
   return check(c);
 }
@@ -447,7 +446,7 @@ void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
   DevScalars<T>* sc = scalars<T>(c);
   int ps_ = prof_open(c, K_EULER);
   auto kern = c->limiter == CSPT_LIMITER_VANLEER ? k_euler_stream<T, ETX, ETY, 1> : k_euler_stream<T, ETX, ETY, 0>;
-  kern<<<grid, ETX * ETY, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN, &sc->smax_bits, &sc->vac_next, zc);
+  kern<<<grid, ETX * ETY, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN, &sc->smax_bits, zc);
   prof_close(c, ps_);
   c->launches++;
 }

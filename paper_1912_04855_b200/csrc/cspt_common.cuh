@@ -84,10 +84,6 @@ template <class T> struct DevScalars {
   T dt;                                  // time step of the step being enqueued
   typename Real<T>::bits_t smax_bits;    // max signal speed, IEEE bits (positive floats order like integers)
   double time;                           // sum of the time steps taken since cspt_set_state
-  // Performance hint only (a wrong value costs time, never correctness): may U^n hold vacuum cells (rho <= rho_vac)?
-  // vac_next is raised by the Euler stage for the U^{n+1} it writes (and by set_state / set_conserved, which do not
-  // look), and becomes vac_cur when the next step's dt kernel runs; kernels take their vacuum shortcuts only then.
-  int vac_cur, vac_next;
 };
 
 // Kernel ids for cspt_profile_* (names in cspt_api.cu, same order).

@@ -119,7 +119,7 @@ template <class T, int TX, int TY, int LIM>
 __global__ void __launch_bounds__(TX* TY, (sizeof(T) == 4 ? 1024 : 512) / (TX * TY))
 k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL, Params<T> P,
                const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, T* __restrict__ UN,
-               typename Real<T>::bits_t* __restrict__ smax_out, int* __restrict__ vac_next, int zchunk) {
+               typename Real<T>::bits_t* __restrict__ smax_out, int zchunk) {
   typedef EulerSmem<T, TX, TY> S;
   extern __shared__ __align__(128) unsigned char sm[];
   uint64_t* bar = (uint64_t*)(sm + S::OFF_BAR);
@@ -135,7 +135,6 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
   constexpr uint32_t TX_BYTES = (uint32_t)((S::U_ELEMS + S::L_ELEMS) * sizeof(T));
 
   if (tid == 0) {
-    *(int*)(bar + 4) = 0;
     mbar_init(&bar[0], 1);
     mbar_init(&bar[1], 1);
     mbar_fence_init();
@@ -155,8 +154,8 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
 
   const T dt = load_dt(sc);
   const T lam = dt * P.inv_h;
-  const bool vac_hint = sc->vac_cur != 0;          // U^n may hold vacuum cells: look for all-vacuum stencils
-  int* vac_seen = (int*)(bar + 4);                 // ... and does the U^{n+1} written here (flag in shared memory)
+  // gas-vacuum shortcuts: in fp32 only (this layout is the fp32 default and the 1024^3 disk is an fp32 workload)
+  constexpr bool VAC = sizeof(T) == 4;
   T Um[5], FPzp[5], acc[5], Utp[5];
   // running maximum of the exact speeds seen by this thread, seeded with the global maximum so far (other
   // CTAs' exact speeds: a lower bound of the final maximum)
@@ -224,7 +223,7 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
       // reconstructed densities lie between theirs, both face velocities are 0 and both flux parts vanish: a warp
       // whose whole in-plane stencil is vacuum skips the reconstruction (most of the 1024^3 disk volume).
       bool vac_xy = false;
-      if (vac_hint) {
+      if (VAC) {
         const T rxy = fmax(fmax(fmax(u_at(0, ty, tx - 1), u_at(0, ty, tx + 1)), fmax(u_at(0, ty - 1, tx), u_at(0, ty + 1, tx))), U0[0]);
         vac_xy = __all_sync(0xffffffffu, !(rxy > P.rho_vac));
       }
@@ -301,7 +300,7 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
 #pragma unroll
       for (int q = 0; q < 5; ++q) Up[q] = sU1[(q * S::UY + (ty + 2)) * S::BX + (tx + S::HX)];
     }
-    if (vac_hint && __all_sync(0xffffffffu, !(fmax(fmax(Um[0], Up[0]), U0[0]) > P.rho_vac))) {
+    if (VAC && __all_sync(0xffffffffu, !(fmax(fmax(Um[0], Up[0]), U0[0]) > P.rho_vac))) {
 #pragma unroll
       for (int q = 0; q < 5; ++q) FPz[q] = FMz[q] = (T)0;         // vacuum along z as well
     } else {
@@ -316,7 +315,6 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
         long long c = L.idx(i, j, p - 1);
 #pragma unroll
         for (int q = 0; q < 5; ++q) UN[c + q * fs] = un[q];
-        if (!(un[0] > P.rho_vac)) *vac_seen = 1;
         // CFL speed of U^{n+1} (G15): exactly rounded, but only for cells whose estimate comes within the
         // filter margin of a speed already known exactly (this thread's maximum or the global one so far);
         // the true maximum always passes the filter, so the result is the exact maximum
@@ -341,8 +339,6 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
     if (tid == 0 && p + 2 <= z1 + 1) issue(p + 2, s);
   }
   block_max_to_global<T>(smax, smax_out);
-  __syncthreads();
-  if (tid == 0 && *vac_seen) atomicOr(vac_next, 1);
 }
 
 }  // namespace cspt

@@ -321,8 +321,6 @@ __global__ void k_dt_finalize(DevScalars<T>* sc, T cfl, T h) {
   T dt = smax > (T)0 ? R::div(R::mul(cfl, h), smax) : R::inf();
   sc->dt = dt;
   sc->smax_bits = 0;
-  sc->vac_cur = sc->vac_next;
-  sc->vac_next = 0;
   if (dt < R::inf()) sc->time += (double)dt;
 }
 
@@ -330,17 +328,13 @@ template <class T>
 __global__ void k_set_dt(DevScalars<T>* sc, T dt) {
   sc->dt = dt;
   sc->smax_bits = 0;
-  sc->vac_cur = sc->vac_next;
-  sc->vac_next = 0;
   sc->time += (double)dt;
 }
 
-// what: bit 0 = new state (time back to 0), bit 1 = the state was written from outside: it may hold vacuum cells
 template <class T>
-__global__ void k_reset_smax(DevScalars<T>* sc, int what) {
+__global__ void k_reset_smax(DevScalars<T>* sc, int reset_time) {
   sc->smax_bits = 0;
-  if (what & 1) sc->time = 0.0;
-  if (what & 2) sc->vac_next = 1;
+  if (reset_time) sc->time = 0.0;
 }
 
 // ---- roofline probe: the FMA rate of the plain FP64 / FP32 pipe, measured on the box the bench runs on ----------
