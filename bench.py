@@ -432,6 +432,7 @@ def run_cspt(args):
     barrier()
     fma_rate = s.probe_fma_rate()        # roofline denominator, measured on this box in this run
     issue_probe = {str(k): s.probe_fma_rate(k) for k in (1, 2, 4, 8)}
+    fma_rate3 = s.probe_fma_rate(-1)     # FMAs with three distinct register operands (register-file bound in fp64)
     barrier()
 
     # ---- timed region: exactly K steps (cspt_run_cfl), device time from CUDA events on the launching stream,
@@ -525,6 +526,7 @@ def run_cspt(args):
                                    % (fma_rate / 148 / ((clocks.get("sm_max_mhz") or 1965) * 1e6), w.dtype,
                                       clocks.get("sm_max_mhz") or 1965),
                     "fma_per_second": fma_rate,
+                    "fma_per_second_three_register_operands": fma_rate3,
                     "fma_per_second_with_other_instructions": issue_probe,
                     "issue_note": "FMA rate with 1 / 2 / 4 / 8 independent integer instructions behind every FMA: cycles per "
                                   "FMA and SMSP ~ max(pipe, 1.1 * (1 + others)), pipe = 2 in fp64 and 1 in fp32 "

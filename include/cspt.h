@@ -154,7 +154,9 @@ int cspt_profile_read(cspt_ctx*, int kid, double* total_ms, long long* launches)
  * 1, 2, 4 or 8: that many independent integer instructions behind every FMA, which shows how the FMAs share the
  * issue port with everything else (an FP64 FMA holds its pipe for two cycles, one other instruction issues in its
  * shadow, every further one costs about one issue cycle: DESIGN.md section 7).  Uses workspace that is dead between
- * steps: call it between steps only.  Syncs.  EINVAL: other_per_fma not one of 0, 1, 2, 4, 8. */
+ * steps: call it between steps only.  Syncs.  other_per_fma = -1: FMAs with three DISTINCT register operands
+ * (x = y * z + x): in fp64 each is a register pair and the register file delivers two pairs per cycle, so these issue
+ * every 3 cycles.  EINVAL: other_per_fma not one of -1, 0, 1, 2, 4, 8. */
 int cspt_probe_fma_rate(cspt_ctx*, int other_per_fma, double* fma_per_second);
 /* ---- z-slab decomposition over several GPUs ("the computational domain is divided between GPUs",
  * :123).  One ctx per slab of nz_local planes; a z face that borders another slab has

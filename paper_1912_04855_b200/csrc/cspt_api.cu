@@ -575,7 +575,8 @@ int probe_fma_t(cspt_ctx* c, int other_per_fma, double* fma_per_second) {
   T* out = field<T>(c, S_ST);
   const int threads = 128, blocks = 148 * 8, iters = other_per_fma ? 1500 : 4000;
   if ((long long)threads * blocks > c->L.fstride * 8) return CSPT_EINVAL;
-  auto kern = other_per_fma == 0   ? k_probe_fma<T, 0>
+  auto kern = other_per_fma < 0    ? k_probe_fma<T, -1>
+              : other_per_fma == 0 ? k_probe_fma<T, 0>
               : other_per_fma == 1 ? k_probe_fma<T, 1>
               : other_per_fma == 2 ? k_probe_fma<T, 2>
               : other_per_fma == 4 ? k_probe_fma<T, 4>
@@ -841,7 +842,7 @@ int cspt_step_filled(cspt_ctx* c, double dt) {
 
 int cspt_probe_fma_rate(cspt_ctx* c, int other_per_fma, double* fma_per_second) {
   if (!c || !fma_per_second) return CSPT_EINVAL;
-  if (other_per_fma != 0 && other_per_fma != 1 && other_per_fma != 2 && other_per_fma != 4 && other_per_fma != 8)
+  if (other_per_fma != -1 && other_per_fma != 0 && other_per_fma != 1 && other_per_fma != 2 && other_per_fma != 4 && other_per_fma != 8)
     return CSPT_EINVAL;
   if (c->cuda_error) return CSPT_ECUDA;
   return DISPATCH(c, probe_fma_t)(c, other_per_fma, fma_per_second);
