@@ -171,8 +171,14 @@ int set_state_t(cspt_ctx* c, const void* rho, const void* u, const void* v, cons
   long long n = (long long)c->L.nx * c->L.ny * c->L.nz;
   T* U = field<T>(c, S_U0);
   T* psi_pad = field<T>(c, S_UT);          // scratch: U~ is dead between steps
+  cudaMemsetAsync(&scalars<T>(c)->has_vac, 0, sizeof(int), c->stream);
   LAUNCH(c, K_IO, k_set_state<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, P, (const T*)rho, (const T*)u, (const T*)v,
-         (const T*)w, (const T*)p, (const T*)psi, U, psi_pad);
+         (const T*)w, (const T*)p, (const T*)psi, U, psi_pad, &scalars<T>(c)->has_vac);
+  // the hint travels to the host without a sync: until it has arrived the variant with the shortcuts runs
+  cudaMemcpyAsync((char*)c->h_pinned + 32, &scalars<T>(c)->has_vac, sizeof(int), cudaMemcpyDeviceToHost, c->stream);
+  cudaEventRecord(c->vac_ev, c->stream);
+  c->vac_pending = true;
+  c->vac_hint = 1;
   fill_ghosts<T>(c, psi_pad, 1, 2);
   fill_ghosts<T>(c, U, 5, 1);
   LAUNCH(c, K_SCALAR, k_reset_smax<T>, 1, 1, scalars<T>(c), 1);
@@ -192,6 +198,8 @@ int set_conserved_t(cspt_ctx* c, const void* const in[5]) {
   T* U = field<T>(c, c->cur ? S_U1 : S_U0);
   for (int f = 0; f < 5; ++f)
     LAUNCH(c, K_IO, k_put_field<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, c->L, (const T*)in[f], U + f * c->L.fstride);
+  c->vac_pending = false;        // the new state was not looked at: keep the shortcuts on
+  c->vac_hint = 1;
   c->smax_valid = false;
   return check(c);
 }
@@ -387,10 +395,10 @@ bool euler1_setup(cspt_ctx* c) {
                               S::BX, S::UY, 5);
   ok = ok && make_field_map(&c->mapL, field<T>(c, S_UT), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 7, S::BX, S::LY, 7);
   if (ok) {
-    ok = cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
-             cudaSuccess &&
-         cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) ==
-             cudaSuccess;
+    ok = cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) == cudaSuccess &&
+         cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) == cudaSuccess &&
+         cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) == cudaSuccess &&
+         cudaFuncSetAttribute(k_euler_stream<T, ETX, ETY, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, S::BYTES) == cudaSuccess;
   }
   return ok;
 }
@@ -434,6 +442,17 @@ void launch_corrector(cspt_ctx* c, const Params<T>& P, const T* U) {
   corr_select<T>(c, &P, U);
 }
 
+// 1: run the kernel variants with the gas-vacuum shortcuts (the state holds vacuum cells, or nobody has looked yet)
+int vacuum_hint(cspt_ctx* c) {
+  if (c->vac_forced >= 0) return c->vac_forced;
+  if (c->vac_pending && cudaEventQuery(c->vac_ev) == cudaSuccess) {
+    c->vac_hint = *(volatile int*)((char*)c->h_pinned + 32) != 0;
+    c->vac_pending = false;
+  }
+  (void)cudaGetLastError();      // cudaErrorNotReady of the query is not an error of the ctx
+  return c->vac_hint;
+}
+
 template <class T>
 void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
   if (c->euler_variant) { euler_select<T>(c, &P, U, UN); return; }
@@ -445,7 +464,9 @@ void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
   dim3 grid(gx, gy, (L.nz + zc - 1) / zc);
   DevScalars<T>* sc = scalars<T>(c);
   int ps_ = prof_open(c, K_EULER);
-  auto kern = c->limiter == CSPT_LIMITER_VANLEER ? k_euler_stream<T, ETX, ETY, 1> : k_euler_stream<T, ETX, ETY, 0>;
+  const bool vl = c->limiter == CSPT_LIMITER_VANLEER, vac = c->step_vac != 0;
+  auto kern = vac ? (vl ? k_euler_stream<T, ETX, ETY, 1, 1> : k_euler_stream<T, ETX, ETY, 0, 1>)
+                  : (vl ? k_euler_stream<T, ETX, ETY, 1, 0> : k_euler_stream<T, ETX, ETY, 0, 0>);
   kern<<<grid, ETX * ETY, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN, &sc->smax_bits, zc);
   prof_close(c, ps_);
   c->launches++;
@@ -453,6 +474,7 @@ void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
 
 template <class T>
 void run_step(cspt_ctx* c, bool fill = true) {
+  if (!c->capturing) c->step_vac = vacuum_hint(c);
   Params<T> P = make_params<T>(c);
   T* U = field<T>(c, c->cur ? S_U1 : S_U0);
   T* UN = field<T>(c, c->cur ? S_U0 : S_U1);
@@ -516,8 +538,10 @@ int capture_two_steps(cspt_ctx* c, double cfl) {
   cudaGraph_t g = nullptr;
   cudaStream_t gs = graph_stream(c), user = c->stream;
   if (!gs) { c->cuda_error = (int)cudaErrorUnknown; return CSPT_ECUDA; }
+  c->step_vac = c->graph_vac = vacuum_hint(c);
   int rc = cuda_call(c, cudaStreamBeginCapture(gs, cudaStreamCaptureModeThreadLocal));
   if (rc) return rc;
+  c->capturing = true;
   const long long l0 = c->launches;
   c->stream = gs;
   for (int s = 0; s < 2; ++s) {
@@ -525,6 +549,7 @@ int capture_two_steps(cspt_ctx* c, double cfl) {
     run_step<T>(c);
   }
   c->stream = user;
+  c->capturing = false;
   c->launches = l0;                                  // counted when the graph is launched
   cudaError_t e = cudaStreamEndCapture(gs, &g);
   if (e != cudaSuccess || !g) { (void)cudaGetLastError(); c->cuda_error = (int)(e ? e : cudaErrorUnknown); return CSPT_ECUDA; }
@@ -542,7 +567,7 @@ int run_cfl_t(cspt_ctx* c, double cfl, int nsteps, double* t_out) {
   if (rc) return rc;
   int left = nsteps;
   if (!c->prof_on && left >= 2) {                    // event pairs cannot be recorded inside a graph: plain loop then
-    if (c->graph[c->cur] && c->graph_cfl != cfl) drop_graphs(c);
+    if ((c->graph[0] || c->graph[1]) && (c->graph_cfl != cfl || c->graph_vac != vacuum_hint(c))) drop_graphs(c);
     if (!c->graph[c->cur]) {
       rc = capture_two_steps<T>(c, cfl);
       if (rc) return rc;
@@ -651,9 +676,15 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->euler_variant = dtype == CSPT_F64 ? 1 : 0;
   if (const char* e = getenv("CSPT_CORR")) c->corr_variant = atoi(e);        // development switches (A/B runs)
   if (const char* e = getenv("CSPT_EULER")) c->euler_variant = atoi(e);
+  c->vac_forced = -1;
+  if (const char* e = getenv("CSPT_VAC")) c->vac_forced = atoi(e) != 0;      // force a variant (tests: both are exact)
   if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
+  if (cudaEventCreateWithFlags(&c->vac_ev, cudaEventDisableTiming) != cudaSuccess) {
+    (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA;
+  }
+  c->vac_hint = 1;
   c->have_maps = dtype == CSPT_F64 ? make_maps<double>(c) : make_maps<float>(c);
-  if (!c->have_maps) { (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }
+  if (!c->have_maps) { (void)cudaGetLastError(); cudaEventDestroy(c->vac_ev); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }
 
   *out = c;
   return CSPT_OK;
@@ -664,6 +695,7 @@ void cspt_destroy(cspt_ctx* c) {
   drop_graphs(c);
   if (c->gstream) cudaStreamDestroy(c->gstream);
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
+  if (c->vac_ev) cudaEventDestroy(c->vac_ev);
   for (int i = 0; i < 2 * c->prof_cap; ++i) cudaEventDestroy(c->prof_ev[i]);
   delete[] c->prof_ev;
   delete[] c->prof_kid;

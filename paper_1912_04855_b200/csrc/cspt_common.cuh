@@ -84,6 +84,7 @@ template <class T> struct DevScalars {
   T dt;                                  // time step of the step being enqueued
   typename Real<T>::bits_t smax_bits;    // max signal speed, IEEE bits (positive floats order like integers)
   double time;                           // sum of the time steps taken since cspt_set_state
+  int has_vac;                           // did cspt_set_state see a cell with rho <= rho_vac (hint for the host, below)
 };
 
 // Kernel ids for cspt_profile_* (names in cspt_api.cu, same order).
@@ -105,7 +106,16 @@ struct cspt_ctx {
   bool smax_valid;         // smax_bits on the device belongs to the current U^n
   int cuda_error;          // sticky
   long long launches;
-  void* h_pinned;          // small pinned staging buffer (scalars)
+  void* h_pinned;          // small pinned staging buffer (scalars; byte 32: has_vac of the last cspt_set_state)
+  // Gas-vacuum hint (performance only, both kernel variants are exact): cspt_set_state counts nothing but notes whether
+  // the state holds vacuum cells; the flag reaches the host asynchronously (vac_ev), and until it has, or after
+  // cspt_set_conserved, the variant WITH the vacuum shortcuts runs.
+  cudaEvent_t vac_ev;
+  bool vac_pending;        // a copy of has_vac is in flight
+  int vac_hint;            // 1: run the kernels with the shortcuts
+  int vac_forced;          // development switch CSPT_VAC: -1 = follow the hint, 0 / 1 = force the variant
+  int step_vac;            // the hint the step being enqueued (or captured) uses
+  bool capturing;          // inside cspt_run_cfl's stream capture
   size_t elem;             // sizeof(T)
   // workspace sub-buffers (byte offsets)
   size_t off_fields, off_inflow, off_scalars;
@@ -122,6 +132,7 @@ struct cspt_ctx {
   cudaGraphExec_t graph[2];
   cudaStream_t gstream;             // capture / replay stream of a ctx that lives on the legacy default stream
   double graph_cfl;                 // the CFL number the graphs were captured with
+  int graph_vac;                    // the vacuum hint the graphs were captured with
   // per-kernel device timing (cspt_profile_*): event pairs recorded around each launch
   bool prof_on;
   int prof_used;                    // pairs recorded since the last reset

@@ -115,7 +115,8 @@ struct EulerSmem {
   static constexpr int BYTES = OFF_BAR + 64 + 128;  // + slack for the 128-byte alignment of the base
 };
 
-template <class T, int TX, int TY, int LIM>
+// VAC = 1: with the gas-vacuum shortcuts (chosen by the host from the hint of cspt_set_state; both variants are exact)
+template <class T, int TX, int TY, int LIM, int VAC>
 __global__ void __launch_bounds__(TX* TY, (sizeof(T) == 4 ? 1024 : 512) / (TX * TY))
 k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL, Params<T> P,
                const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, T* __restrict__ UN,
@@ -154,8 +155,6 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
 
   const T dt = load_dt(sc);
   const T lam = dt * P.inv_h;
-  // gas-vacuum shortcuts: in fp32 only (this layout is the fp32 default and the 1024^3 disk is an fp32 workload)
-  constexpr bool VAC = sizeof(T) == 4;
   T Um[5], FPzp[5], acc[5], Utp[5];
   // running maximum of the exact speeds seen by this thread, seeded with the global maximum so far (other
   // CTAs' exact speeds: a lower bound of the final maximum)

@@ -93,16 +93,18 @@ template <> struct Fast<float> {
 template <class T>
 __global__ void k_set_state(Params<T> P, const T* __restrict__ rho, const T* __restrict__ u,
                             const T* __restrict__ v, const T* __restrict__ w, const T* __restrict__ p,
-                            const T* __restrict__ psi, T* __restrict__ U, T* __restrict__ psi_pad) {
+                            const T* __restrict__ psi, T* __restrict__ U, T* __restrict__ psi_pad, int* __restrict__ has_vac) {
   typedef Real<T> R;
   const Layout& L = P.L;
   long long n = (long long)L.nx * L.ny * L.nz;
+  int vac = 0;
   for (long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) {
     int i = (int)(m % L.nx);
     long long r = m / L.nx;
     int j = (int)(r % L.ny), k = (int)(r / L.ny);
     long long c = L.idx(i, j, k);
     T ro = rho[m], uu = u[m], vv = v[m], ww = w[m];
+    vac |= !(ro > P.rho_vac);
     U[c] = ro;
     U[c + L.fstride] = R::mul(ro, uu);
     U[c + 2 * L.fstride] = R::mul(ro, vv);
@@ -111,6 +113,7 @@ __global__ void k_set_state(Params<T> P, const T* __restrict__ rho, const T* __r
     U[c + 4 * L.fstride] = R::add(R::div(p[m], R::sub(P.gamma, (T)1)), R::mul(R::mul((T)0.5, ro), ke));
     if (psi_pad) psi_pad[c] = psi[m];
   }
+  if (__syncthreads_or(vac) && threadIdx.x == 0) atomicOr(has_vac, 1);     // hint for the host: vacuum shortcuts pay
 }
 
 template <class T>

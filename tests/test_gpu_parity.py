@@ -284,6 +284,31 @@ def test_kernel_switch_discards_the_state_and_rejects_unknown_values(cspt, oracl
 
 
 # ---- degenerate cases ---------------------------------------------------------------------------
+def test_vacuum_shortcuts_are_exact(cspt, oracle_mod, monkeypatch):
+    """The fp32 Euler stage exists with and without the gas-vacuum shortcuts (chosen by a host-side hint from
+    cspt_set_state); both must give the same bits, on a workload with vacuum and on one without."""
+    for w in (wl.disk(n=48), wl.random_smooth(40, 24, 20, dtype="f32")):
+        got = []
+        for force in ("0", "1"):
+            monkeypatch.setenv("CSPT_VAC", force)
+            s = make_solver(cspt, w)
+            s.set_state(*w.fields())
+            s.run_cfl(w.cfl, 6)
+            s.step_cfl(w.cfl)
+            got.append([t.cpu().numpy() for t in s.get_conserved()])
+            s.close()
+        monkeypatch.delenv("CSPT_VAC")
+        for a, b in zip(*got):
+            assert np.array_equal(a, b)
+        hinted = make_solver(cspt, w)                    # no override: the hint picks one of the two
+        hinted.set_state(*w.fields())
+        hinted.run_cfl(w.cfl, 6)
+        hinted.step_cfl(w.cfl)
+        for a, b in zip(got[0], [t.cpu().numpy() for t in hinted.get_conserved()]):
+            assert np.array_equal(a, b)
+        hinted.close()
+
+
 def test_all_vacuum_grid(cspt, oracle_mod):
     import torch
     z = np.zeros((4, 4, 8))
