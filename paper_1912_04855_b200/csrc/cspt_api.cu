@@ -419,7 +419,9 @@ bool make_maps(cspt_ctx* c) {
   return ok;
 }
 
-// primitives + HFC/SUL{predictor} over the extended domain interior(+)2
+// primitives + HFC/SUL{predictor} over the extended domain interior(+)2: 32 x 4 tiles, inputs through a TMA ring of two
+// stages (3.78 -> 3.14 ms in fp64, 2.04 -> 1.75 ms in fp32 against the register prefetch; deeper rings and 32 x 8 tiles
+// measured slower, profiles/r2_kernels.md)
 constexpr int PTX = 32, PTY = 4;
 template <class T>
 void launch_predictor(cspt_ctx* c, const Params<T>& P, const T* U) {
@@ -430,10 +432,32 @@ void launch_predictor(cspt_ctx* c, const Params<T>& P, const T* U) {
   int zc = pick_zchunk(gx * gy, L.nz + 4);
   dim3 grid(gx, gy, (L.nz + 4 + zc - 1) / zc);
   int ps_ = prof_open(c, K_PREDICTOR);
-  k_predictor_stream<T, PTX, PTY><<<grid, PTX * PTY, 0, c->stream>>>(P, scalars<T>(c), U, field<T>(c, S_F),
-                                                                      field<T>(c, S_ST), zc, x0, x1);
+  auto launch = [&](auto kern, int bytes) {
+    kern<<<grid, PTX * PTY, bytes, c->stream>>>(c->mapPU[c->cur], c->mapPF, P, scalars<T>(c), U, field<T>(c, S_F),
+                                                 field<T>(c, S_ST), zc, x0, x1);
+  };
+  if (c->pred_stages == 2) launch(k_predictor_stream<T, PTX, PTY, 2>, PredRing<T, PTX, PTY, 2>::BYTES);
+  else if (c->pred_stages == 3) launch(k_predictor_stream<T, PTX, PTY, 3>, PredRing<T, PTX, PTY, 3>::BYTES);
+  else launch(k_predictor_stream<T, PTX, PTY, 0>, 0);
   prof_close(c, ps_);
   c->launches++;
+}
+
+// TMA views of the predictor's inputs (cspt_lagrange.cuh, PredRing) and the dynamic shared memory of its ring
+template <class T>
+bool predictor_setup(cspt_ctx* c) {
+  const Layout& L = c->L;
+  typedef PredRing<T, PTX, PTY, 2> R;
+  bool ok = true;
+  for (int b = 0; b < 2; ++b)
+    ok = ok && make_field_map(&c->mapPU[b], field<T>(c, b ? S_U1 : S_U0), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 5,
+                              R::BXT, PTY + 2, 5);
+  ok = ok && make_field_map(&c->mapPF, field<T>(c, S_F), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 3, R::BXT, PTY, 3);
+  ok = ok && cudaFuncSetAttribute(k_predictor_stream<T, PTX, PTY, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                  PredRing<T, PTX, PTY, 2>::BYTES) == cudaSuccess &&
+       cudaFuncSetAttribute(k_predictor_stream<T, PTX, PTY, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            PredRing<T, PTX, PTY, 3>::BYTES) == cudaSuccess;
+  return ok;
 }
 
 // HFC/SUL{corrector} over the extended domain interior(+)1
@@ -676,6 +700,8 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->euler_variant = dtype == CSPT_F64 ? 1 : 0;
   if (const char* e = getenv("CSPT_CORR")) c->corr_variant = atoi(e);        // development switches (A/B runs)
   if (const char* e = getenv("CSPT_EULER")) c->euler_variant = atoi(e);
+  c->pred_stages = 2;
+  if (const char* e = getenv("CSPT_PRED")) c->pred_stages = atoi(e);          // 0: register prefetch, 2 | 3: TMA ring depth
   c->vac_forced = -1;
   if (const char* e = getenv("CSPT_VAC")) c->vac_forced = atoi(e) != 0;      // force a variant (tests: both are exact)
   if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
@@ -683,7 +709,8 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
     (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA;
   }
   c->vac_hint = 1;
-  c->have_maps = dtype == CSPT_F64 ? make_maps<double>(c) : make_maps<float>(c);
+  c->have_maps = dtype == CSPT_F64 ? (make_maps<double>(c) && predictor_setup<double>(c))
+                                   : (make_maps<float>(c) && predictor_setup<float>(c));
   if (!c->have_maps) { (void)cudaGetLastError(); cudaEventDestroy(c->vac_ev); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }
 
   *out = c;

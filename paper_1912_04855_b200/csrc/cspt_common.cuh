@@ -122,6 +122,8 @@ struct cspt_ctx {
   long long inflow_plane;  // elements per captured plane
   // TMA views (x, y, z, field) of the two U buffers, of the (U~, xi) group and of the star group
   CUtensorMap mapU[2], mapL, mapS;
+  CUtensorMap mapPU[2], mapPF;      // predictor: U^n (tile + halo 1) and f (tile)
+  int pred_stages;                  // predictor: 0 = register prefetch, 2..4 = TMA ring of that many stages
   bool have_maps;
   int kernel;               // CSPT_KERNEL_*: smoothing kernel W of Eq. (7)
   int limiter;              // CSPT_LIMITER_*: TVD slope of Eq. (8) in the Euler stage

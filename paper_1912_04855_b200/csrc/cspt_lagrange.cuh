@@ -35,8 +35,10 @@ template <> struct Pair<float> { typedef float2 type; static __device__ __forcei
 //   S_c = sum_o a(|o|^2) o_c phi_{i+o},   T = sum_c sum_o a(|o|^2) o_c (phi u_c)_{i+o}
 // (Q_m = -phi_i S / h + rho f,  Q_E = -phi_i (u_i . S + T) / (2h) + rho u_i . f;  G1-G6).
 // One CTA owns a TX x TY column of the extended domain interior(+)2 and streams along z.  Per plane q
-// the threads compute phi, phi u, phi v, phi w of the (TX+2) x (TY+2) cells straight from U^n in
-// global memory into a 2-slot shared-memory buffer; every thread then forms the IN-PLANE parts of the
+// one TMA box of U^n (tile + halo 1) and one of f land in a two-stage shared-memory ring, two planes ahead of their
+// use (PredRing; the earlier version loaded them into registers one plane ahead and spent 19 % of its warp cycles
+// waiting for the first of them and 24 % at the barrier behind it); the threads turn them into phi, phi u, phi v,
+// phi w of the (TX+2) x (TY+2) cells in a 2-slot shared-memory buffer; every thread then forms the IN-PLANE parts of the
 // sums of plane q for its column: with the |o_z| = 1 weights they belong to the particles of planes
 // q-1 and q+1 (sign of the z terms flipped), with the o_z = 0 weights to plane q.  The running sums
 // of the two particles in flight live in registers; particle q-1 is finished (Eq. (5)) when plane q
@@ -63,12 +65,32 @@ struct PredSmem {
   static_assert(NHALO <= TX * TY, "one halo cell per thread at most");
 };
 
-template <class T, int TX, int TY>
+// TMA ring of the predictor's inputs (NSTG > 0): per plane one box of U^n (5 fields, tile + halo 1) and one of f (3
+// fields, tile) land in a stage of dynamic shared memory, NSTG planes ahead of their use; the boxes start on a 16-byte
+// boundary in x (A elements) and are wide enough for the tile whatever the remainder.
+template <class T, int TX, int TY, int NSTG>
+struct PredRing {
+  static constexpr int A = 16 / (int)sizeof(T);
+  static constexpr int BXT = sizeof(T) == 8 ? 36 : 40;
+  static constexpr int U_ELEMS = 5 * (TY + 2) * BXT, F_ELEMS = 3 * TY * BXT;
+  static constexpr int U_BYTES = U_ELEMS * (int)sizeof(T), F_BYTES = F_ELEMS * (int)sizeof(T);
+  static constexpr int OFF_F = (U_BYTES + 127) / 128 * 128;
+  static constexpr int STAGE = (OFF_F + F_BYTES + 127) / 128 * 128;
+  static constexpr int OFF_BAR = NSTG * STAGE;
+  static constexpr int BYTES = NSTG > 0 ? OFF_BAR + 8 * NSTG + 128 : 0;    // + slack for the 128-byte alignment
+};
+
+template <class T, int TX, int TY, int NSTG = 0>
 __global__ void __launch_bounds__(TX* TY, (sizeof(T) == 4 ? 768 : 512) / (TX * TY))
-k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, const T* __restrict__ F,
+k_predictor_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapF, Params<T> P,
+                   const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, const T* __restrict__ F,
                    T* __restrict__ ST, int zchunk, int x0, int x1) {      // particle columns [x0, x1)
   typedef PredSmem<T, TX, TY> S;
+  typedef PredRing<T, TX, TY, NSTG> R;
   __shared__ T sbuf[2][S::PLANE];
+  extern __shared__ unsigned char ring_raw[];
+  unsigned char* ring = (unsigned char*)(((uintptr_t)ring_raw + 127) & ~(uintptr_t)127);
+  uint64_t* bar = (uint64_t*)(ring + R::OFF_BAR);
   const Layout& L = P.L;
   const int tid = threadIdx.x, tx = tid % TX, ty = tid / TX;
   const int i0 = x0 + (int)blockIdx.x * TX, j0 = -2 + (int)blockIdx.y * TY;
@@ -97,11 +119,32 @@ k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* _
     sb[3 * S::BY * S::BX + o] = q.phi * q.w;
   };
 
+  // TMA ring: box start (padded x index rounded down to a 16-byte boundary) and this thread's columns inside the box
+  const int bxs = ((i0 - 1 + GX) / R::A) * R::A, lxo = (i0 - 1 + GX) - bxs;
+  auto slot_of = [&](int qq) { return (qq - (z0 - 1)) % (NSTG > 0 ? NSTG : 1); };
+  auto issue = [&](int qq) {
+    const int k = slot_of(qq);
+    mbar_expect_tx(&bar[k], (uint32_t)(R::U_BYTES + R::F_BYTES));
+    tma_load_4d(ring + k * R::STAGE, &mapU, &bar[k], bxs, j0 - 1 + NG, qq + NG, 0);
+    tma_load_4d(ring + k * R::STAGE + R::OFF_F, &mapF, &bar[k], bxs, j0 + NG, qq + NG, 0);
+  };
+  uint32_t phase = 0;
   T Uo[5], Uh[5];                 // plane q: own and halo cell, loaded one iteration ahead
-  {
+  if (NSTG == 0) {
     const long long co = c_own + (long long)(z0 - 1) * sz, ch = c_halo + (long long)(z0 - 1) * sz;
 #pragma unroll
     for (int f = 0; f < 5; ++f) { Uo[f] = __ldg(U + co + f * fs); Uh[f] = has_halo ? __ldg(U + ch + f * fs) : (T)0; }
+  } else {
+    if (tid == 0) {
+#pragma unroll
+      for (int k = 0; k < NSTG; ++k) mbar_init(&bar[k], 1);
+      mbar_fence_init();
+      prefetch_tmap(&mapU);
+      prefetch_tmap(&mapF);
+    }
+    __syncthreads();
+    if (tid == 0)
+      for (int qq = z0 - 1; qq < z0 - 1 + NSTG && qq <= z1; ++qq) issue(qq);
   }
   // periodic x (x0 == 0: interior columns only): the ghost columns -2, -1, nx, nx+1 hold what this kernel would
   // compute there, i.e. the value of the column they wrap onto (same inputs, same arithmetic); woff[g] is the
@@ -119,6 +162,21 @@ k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* _
 
   for (int q = z0 - 1; q <= z1; ++q) {
     T* sb = sbuf[(q - (z0 - 1)) & 1];
+    T fstage[3] = {0, 0, 0};
+    if (NSTG > 0) {               // plane q has landed: own and halo cell of U^n, f of particle q
+      const int k = slot_of(q);
+      mbar_wait(&bar[k], (phase >> k) & 1u);
+      phase ^= 1u << k;
+      const T* sU = (const T*)(ring + k * R::STAGE);
+      const T* sF = (const T*)(ring + k * R::STAGE + R::OFF_F);
+#pragma unroll
+      for (int f = 0; f < 5; ++f) {
+        Uo[f] = sU[(f * (TY + 2) + ty + 1) * R::BXT + lxo + 1 + tx];
+        Uh[f] = has_halo ? sU[(f * (TY + 2) + hy + 1) * R::BXT + lxo + 1 + hx] : (T)0;
+      }
+#pragma unroll
+      for (int f = 0; f < 3; ++f) fstage[f] = sF[(f * TY + ty) * R::BXT + lxo + 1 + tx];
+    }
     // O1 for plane q
     Prim<T> po = prim_quick<T>(Uo[0], Uo[1], Uo[2], Uo[3], Uo[4], P.gamma, P.rho_vac);
     put(sb, ty, tx, po);
@@ -133,7 +191,10 @@ k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* _
     T fq[3];
 #pragma unroll
     for (int f = 0; f < 3; ++f) fq[f] = fn[f];
-    if (q < z1) {
+    if (NSTG > 0) {
+#pragma unroll
+      for (int f = 0; f < 3; ++f) fn[f] = fstage[f];
+    } else if (q < z1) {
       const long long co = c_own + (long long)(q + 1) * sz, ch = c_halo + (long long)(q + 1) * sz;
 #pragma unroll
       for (int f = 0; f < 5; ++f) { Uo[f] = __ldg(U + co + f * fs); if (has_halo) Uh[f] = __ldg(U + ch + f * fs); }
@@ -145,6 +206,7 @@ k_predictor_stream(Params<T> P, const DevScalars<T>* __restrict__ sc, const T* _
     }
     const long long cs = c_own + (long long)(q - 1) * sz;       // particle q-1
     __syncthreads();
+    if (NSTG > 0 && tid == 0 && q + NSTG <= z1) issue(q + NSTG);   // everyone has read stage q
 
     // in-plane parts of the lattice sums of plane q (tile coordinates of the own column: tx, ty)
     auto at = [&](int f, int oy, int ox) { return sb[(f * S::BY + (ty + 1 + oy)) * S::BX + (tx + 1 + ox)]; };
