@@ -297,10 +297,10 @@ def stored_traffic(w, kernel):
             d = json.load(fh)
         e = d.get("%s %dx%dx%d %s" % (w.name, w.nx, w.ny, w.nz, w.dtype))
         if e and e.get("sources_sha") == sources_sha():
-            return e.get(kernel), e.get("source")
+            return e.get(kernel), e.get("source"), (e.get("ncu") or {}).get(kernel)
     except Exception:
         pass
-    return None, None
+    return None, None, None
 
 
 def device_fields(w, device):
@@ -506,7 +506,7 @@ def run_cspt(args):
     words = KERNEL_WORDS.get(dom, MIN_WORDS_PER_CELL)
     dom_bytes = words * esz * w.cells
     ach = dom_bytes / (dom_ms * 1e-3) / 1e9
-    traffic, traffic_src = stored_traffic(w, dom)
+    traffic, traffic_src, ncu_stored = stored_traffic(w, dom)
     hbm = {"achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": peak_src,
            "algorithmic_bytes_per_launch": dom_bytes}
     share = (prof[dom][0] / args.steps) / prof_step_ms
@@ -521,7 +521,7 @@ def run_cspt(args):
                     "instr_frac": ALGO_INSTR[dom] * w.cells / (dom_ms * 1e-3) / fma_rate,
                     "instr_frac_is": "SURVEY 8(d) instruction list (%d FP instructions per cell, FMA counted once) over "
                                      "the measured instruction rate of the pipe" % ALGO_INSTR[dom],
-                    "traffic": traffic, "traffic_source": traffic_src,
+                    "traffic": traffic, "traffic_source": traffic_src, "ncu": ncu_stored,
                     "peak_source": "measured in this run: cspt_probe_fma_rate, %.1f %s FMA per clock per SM at %d MHz"
                                    % (fma_rate / 148 / ((clocks.get("sm_max_mhz") or 1965) * 1e6), w.dtype,
                                       clocks.get("sm_max_mhz") or 1965),
@@ -535,7 +535,7 @@ def run_cspt(args):
                     "algorithmic_instr_per_cell": ALGO_INSTR[dom], "kernel_ms": dom_ms, "share_of_step": share,
                     "hbm": hbm}
     else:
-        roofline = dict(hbm, bound="hbm", kernel=dom, traffic=traffic, traffic_source=traffic_src, kernel_ms=dom_ms,
+        roofline = dict(hbm, bound="hbm", kernel=dom, traffic=traffic, traffic_source=traffic_src, ncu=ncu_stored, kernel_ms=dom_ms,
                         share_of_step=share)
     step_ach = MIN_WORDS_PER_CELL * esz * w.cells / (step_ms * 1e-3) / 1e9
     step_hbm = {"bytes_per_cell_update": MIN_WORDS_PER_CELL * esz, "achieved_gbs": step_ach, "frac_of_measured": step_ach / peak,
