@@ -496,20 +496,23 @@ def run_cspt(args):
     # ---- roofline of the dominant kernel, from the event pairs of the profiled pass
     peak, peak_src = peaks()
     step_ms = tmax / args.steps
+    # the library records a bounded number of event pairs (8192): with very many steps the profiled pass covers only
+    # the first ones, so every per-step figure is taken over the steps that WERE recorded (the Euler stage runs once
+    # per step and is the last launch of a step)
+    prof_steps = min(args.steps, int(prof.get("euler", (0, args.steps))[1])) or args.steps
     kern = {}
     for k, v in prof.items():
-        per_step = v[1] / args.steps
-        kern[k] = {"ms_per_step": v[0] / args.steps, "launches_per_step": per_step}
+        kern[k] = {"ms_per_step": v[0] / prof_steps, "launches_per_step": v[1] / prof_steps}
     dom = max(prof.items(), key=lambda kv: kv[1][0])[0]
     dom_ms = prof[dom][0] / prof[dom][1]
-    prof_step_ms = sum(v[0] for v in prof.values()) / args.steps
+    prof_step_ms = sum(v[0] for v in prof.values()) / prof_steps
     words = KERNEL_WORDS.get(dom, MIN_WORDS_PER_CELL)
     dom_bytes = words * esz * w.cells
     ach = dom_bytes / (dom_ms * 1e-3) / 1e9
     traffic, traffic_src, ncu_stored = stored_traffic(w, dom)
     hbm = {"achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "peak_source": peak_src,
            "algorithmic_bytes_per_launch": dom_bytes}
-    share = (prof[dom][0] / args.steps) / prof_step_ms
+    share = (prof[dom][0] / prof_steps) / prof_step_ms
     if dom in ALGO_FLOPS and args.kernel == "cubic":
         # the corrector is bound by the plain FP64 / FP32 pipe.  Denominator: the FMA rate
         # cspt_probe_fma_rate measured in THIS run just before the timed region (thread-level FMA/s; an FP instruction
@@ -549,7 +552,7 @@ def run_cspt(args):
                        api="cspt_run_cfl"),
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "kernels": kern,
         "kernels_note": "per-kernel times from a second pass of the same K steps with an event pair around every launch "
-                        "(%.3f ms per step in that pass)" % prof_step_ms,
+                        "(%.3f ms per step in that pass, %d steps recorded)" % (prof_step_ms, prof_steps),
         "roofline": roofline, "step_hbm": step_hbm,
     }
 
