@@ -60,7 +60,7 @@ def parse():
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
                     help="N > 1: independent replicas (default; north_star has no domain decomposition) or ONE grid cut "
                          "into z slabs over the ranks (SURVEY 8(f) NEXT-2, strong scaling)")
-    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--e2e-steps", type=int, default=8)
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config throughput table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -471,19 +471,23 @@ def run_cspt(args):
     s.step_cfl(w.cfl)
     s.get_conserved_host(out)           # warm-up of the host path
     barrier()
+    # asynchronous host entry points: the result of one step leaves on one copy stream while the input of the next
+    # arrives on another (both directions of the host link); every step still copies its own inputs and its own result
     f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     f0.record(s.stream)
     for _ in range(n_e2e):
-        s.set_state_host(*fields)
+        s.set_state_host_async(*fields)
         s.step_cfl(w.cfl)
-        s.get_conserved_host(out)
+        s.get_conserved_host_async(out)
+    s.sync()                            # the ctx's stream and both copy streams
     f1.record(s.stream)
     barrier()
     ems = f0.elapsed_time(f1)
     ems = max_over_ranks(ems, world, "cuda")
     e2e = {"value": job_value(w.cells, n_e2e, world, ems), "unit": UNIT,
            "h2d_bytes_per_step": 6 * w.cells * esz, "d2h_bytes_per_step": 5 * w.cells * esz, "steps": n_e2e,
-           "what": "cspt_set_state_host + cspt_step_cfl + cspt_get_conserved_host per step, pinned host buffers"}
+           "what": "cspt_set_state_host_async + cspt_step_cfl + cspt_get_conserved_host_async per step, one cspt_sync at the "
+                   "end, pinned host buffers (the copy out of step k overlaps the copy in of step k+1)"}
     s.close()
     del s, out, fields
     torch.cuda.empty_cache()

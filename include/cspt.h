@@ -73,6 +73,12 @@ int cspt_set_state(cspt_ctx*, const void* rho, const void* u, const void* v, con
 /* Same, from HOST buffers (copied through the stream; syncs). */
 int cspt_set_state_host(cspt_ctx*, const void* rho, const void* u, const void* v, const void* w,
                         const void* p, const void* psi);
+/* The same without the final wait: the six copies run on a copy stream of the ctx, the kernels follow on the ctx's
+ * stream.  The host arrays (pinned, else the copies are not asynchronous) must stay untouched until cspt_sync.  With
+ * cspt_get_conserved_host_async this lets the result of one state leave while the next state arrives (both
+ * directions of the host link at once).  Does not sync. */
+int cspt_set_state_host_async(cspt_ctx*, const void* rho, const void* u, const void* v, const void* w,
+                              const void* p, const void* psi);
 
 /* CFL time step (paper silent; reading G15): dt = cfl*h / max_cells(c + max(|u|,|v|,|w|)),
  * c = sqrt(gamma p / rho), vacuum cells skipped; +inf if every cell is vacuum.
@@ -130,6 +136,10 @@ int cspt_get_state(cspt_ctx*, void* rho, void* u, void* v, void* w, void* p);
 int cspt_get_conserved(cspt_ctx*, void* rho, void* mx, void* my, void* mz, void* E);
 /* Same, into HOST buffers (syncs). */
 int cspt_get_conserved_host(cspt_ctx*, void* rho, void* mx, void* my, void* mz, void* E);
+/* The same without the final wait: the five fields are staged on the device and copied out on a second copy stream;
+ * the host arrays hold the result after cspt_sync (which waits for the ctx's stream and both copy streams).  A later
+ * step waits by itself until the staged result has left.  Does not sync. */
+int cspt_get_conserved_host_async(cspt_ctx*, void* rho, void* mx, void* my, void* mz, void* E);
 /* Overwrites the conserved variables, keeping psi/f and the captured inflow layers
  * (checkpoint restore).  Device pointers. */
 int cspt_set_conserved(cspt_ctx*, const void* rho, const void* mx, const void* my, const void* mz,
@@ -187,7 +197,7 @@ int cspt_fill_ghosts(cspt_ctx*);
 int cspt_step_filled(cspt_ctx*, double dt);
 /* The cudaError_t value behind a CSPT_ECUDA status of this ctx (0 if none). */
 int cspt_cuda_error(const cspt_ctx*);
-/* Waits for the ctx's stream. */
+/* Waits for the ctx's stream and for the copy streams of the *_host_async calls. */
 int cspt_sync(cspt_ctx*);
 /* Frees the ctx, never the workspace.  NULL is allowed. */
 void cspt_destroy(cspt_ctx*);

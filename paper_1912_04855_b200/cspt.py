@@ -25,6 +25,7 @@ SYMBOLS = [
     ("cspt_create", _ci, [ctypes.POINTER(_vp), _ci, _ci, _ci, _cd, _cd, ctypes.POINTER(_ci), _ci, _vp, _sz, _vp]),
     ("cspt_set_state", _ci, [_vp] * 7),
     ("cspt_set_state_host", _ci, [_vp] * 7),
+    ("cspt_set_state_host_async", _ci, [_vp] * 7),
     ("cspt_compute_dt", _ci, [_vp, _cd, _pd]),
     ("cspt_set_kernel", _ci, [_vp, _ci]),
     ("cspt_set_limiter", _ci, [_vp, _ci]),
@@ -35,6 +36,7 @@ SYMBOLS = [
     ("cspt_get_state", _ci, [_vp] * 6),
     ("cspt_get_conserved", _ci, [_vp] * 6),
     ("cspt_get_conserved_host", _ci, [_vp] * 6),
+    ("cspt_get_conserved_host_async", _ci, [_vp] * 6),
     ("cspt_set_conserved", _ci, [_vp] * 6),
     ("cspt_get_vacuum_mask", _ci, [_vp, _vp]),
     ("cspt_launch_count", ctypes.c_longlong, [_vp]),
@@ -162,6 +164,11 @@ class Solver:
         ts = [self._host(a) for a in (rho, u, v, w, p, psi)]
         _check(lib().cspt_set_state_host(self._h, *[_dptr(t) for t in ts]), "cspt_set_state_host")
 
+    def set_state_host_async(self, rho, u, v, w, p, psi):
+        """Enqueues only: the (pinned) host tensors must stay untouched until sync()."""
+        ts = [self._host(a) for a in (rho, u, v, w, p, psi)]
+        _check(lib().cspt_set_state_host_async(self._h, *[_dptr(t) for t in ts]), "cspt_set_state_host_async")
+
     def compute_dt(self, cfl):
         out = ctypes.c_double()
         _check(lib().cspt_compute_dt(self._h, float(cfl), ctypes.byref(out)), "cspt_compute_dt")
@@ -213,6 +220,12 @@ class Solver:
     def get_conserved_host(self, out):
         ts = [self._host(a) for a in out]
         _check(lib().cspt_get_conserved_host(self._h, *[_dptr(t) for t in ts]), "cspt_get_conserved_host")
+        return out
+
+    def get_conserved_host_async(self, out):
+        """Enqueues only: `out` holds the result after sync()."""
+        ts = [self._host(a) for a in out]
+        _check(lib().cspt_get_conserved_host_async(self._h, *[_dptr(t) for t in ts]), "cspt_get_conserved_host_async")
         return out
 
     def set_conserved(self, rho, mx, my, mz, E):

@@ -496,8 +496,17 @@ void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
   c->launches++;
 }
 
+// a result on its way to the host (cspt_get_conserved_host_async) is staged in the U~ / xi slots: a step waits for it
+void wait_pending_output(cspt_ctx* c) {
+  if (c->out_pending && !c->capturing) {
+    cudaStreamWaitEvent(c->stream, c->ev_out_done, 0);
+    c->out_pending = false;
+  }
+}
+
 template <class T>
 void run_step(cspt_ctx* c, bool fill = true) {
+  wait_pending_output(c);
   if (!c->capturing) c->step_vac = vacuum_hint(c);
   Params<T> P = make_params<T>(c);
   T* U = field<T>(c, c->cur ? S_U1 : S_U0);
@@ -586,6 +595,7 @@ int capture_two_steps(cspt_ctx* c, double cfl) {
 
 template <class T>
 int run_cfl_t(cspt_ctx* c, double cfl, int nsteps, double* t_out) {
+  wait_pending_output(c);
   ensure_smax<T>(c);
   int rc = check(c);
   if (rc) return rc;
@@ -650,6 +660,19 @@ int probe_fma_t(cspt_ctx* c, int other_per_fma, double* fma_per_second) {
 // dense staging arrays for the *_host entry points live in the (dead between steps)
 // star-group slots S_ST.. (8 padded slots >= 6 dense arrays)
 template <class T> T* staging(cspt_ctx* c, int f) { return field<T>(c, S_ST + f); }
+// staging of cspt_get_conserved_host_async: the U~ (but the first, psi's scratch) and xi slots, dead between steps and
+// untouched by cspt_set_state, so that the next input can be staged while the result is still on its way out
+template <class T> T* staging_out(cspt_ctx* c, int f) { return field<T>(c, S_UT + 1 + f); }
+
+bool ensure_copy_streams(cspt_ctx* c) {
+  if (c->h2d_stream) return true;
+  bool ok = cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking) == cudaSuccess;
+  cudaEvent_t* ev[4] = {&c->ev_in_free, &c->ev_in_ready, &c->ev_out_ready, &c->ev_out_done};
+  for (int k = 0; ok && k < 4; ++k) ok = cudaEventCreateWithFlags(ev[k], cudaEventDisableTiming) == cudaSuccess;
+  if (!ok) { (void)cudaGetLastError(); c->cuda_error = (int)cudaErrorUnknown; }
+  return ok;
+}
 
 }  // namespace
 
@@ -723,6 +746,10 @@ void cspt_destroy(cspt_ctx* c) {
   if (c->gstream) cudaStreamDestroy(c->gstream);
   if (c->h_pinned) cudaFreeHost(c->h_pinned);
   if (c->vac_ev) cudaEventDestroy(c->vac_ev);
+  if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
+  if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
+  for (cudaEvent_t e : {c->ev_in_free, c->ev_in_ready, c->ev_out_ready, c->ev_out_done})
+    if (e) cudaEventDestroy(e);
   for (int i = 0; i < 2 * c->prof_cap; ++i) cudaEventDestroy(c->prof_ev[i]);
   delete[] c->prof_ev;
   delete[] c->prof_kid;
@@ -794,6 +821,27 @@ int cspt_set_state_host(cspt_ctx* c, const void* rho, const void* u, const void*
   int rc = DISPATCH(c, set_state_t)(c, dev[0], dev[1], dev[2], dev[3], dev[4], dev[5]);
   if (rc) return rc;
   return cuda_call(c, cudaStreamSynchronize(c->stream));
+}
+
+int cspt_set_state_host_async(cspt_ctx* c, const void* rho, const void* u, const void* v, const void* w, const void* p,
+                              const void* psi) {
+  if (!c || !rho || !u || !v || !w || !p || !psi) return CSPT_EINVAL;
+  if (c->cuda_error) return CSPT_ECUDA;
+  if (!ensure_copy_streams(c)) return CSPT_ECUDA;
+  const void* in[6] = {rho, u, v, w, p, psi};
+  void* dev[6];
+  size_t bytes = (size_t)c->L.nx * c->L.ny * c->L.nz * c->elem;
+  // the staging slots are the star group of the last step: the copies start when the work enqueued so far is done
+  int rc = cuda_call(c, cudaEventRecord(c->ev_in_free, c->stream));
+  if (!rc) rc = cuda_call(c, cudaStreamWaitEvent(c->h2d_stream, c->ev_in_free, 0));
+  for (int f = 0; f < 6 && !rc; ++f) {
+    dev[f] = c->dtype == CSPT_F64 ? (void*)staging<double>(c, f) : (void*)staging<float>(c, f);
+    rc = cuda_call(c, cudaMemcpyAsync(dev[f], in[f], bytes, cudaMemcpyHostToDevice, c->h2d_stream));
+  }
+  if (!rc) rc = cuda_call(c, cudaEventRecord(c->ev_in_ready, c->h2d_stream));
+  if (!rc) rc = cuda_call(c, cudaStreamWaitEvent(c->stream, c->ev_in_ready, 0));
+  if (rc) return rc;
+  return DISPATCH(c, set_state_t)(c, dev[0], dev[1], dev[2], dev[3], dev[4], dev[5]);
 }
 
 int cspt_compute_dt(cspt_ctx* c, double cfl, double* dt_host_out) {
@@ -939,6 +987,27 @@ int cspt_get_conserved_host(cspt_ctx* c, void* rho, void* mx, void* my, void* mz
   return cuda_call(c, cudaStreamSynchronize(c->stream));
 }
 
+int cspt_get_conserved_host_async(cspt_ctx* c, void* rho, void* mx, void* my, void* mz, void* E) {
+  if (!c || !rho || !mx || !my || !mz || !E) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  if (!ensure_copy_streams(c)) return CSPT_ECUDA;
+  wait_pending_output(c);                     // an earlier result still leaving through the same staging slots
+  void* host[5] = {rho, mx, my, mz, E};
+  void* dev[5];
+  for (int f = 0; f < 5; ++f) dev[f] = c->dtype == CSPT_F64 ? (void*)staging_out<double>(c, f) : (void*)staging_out<float>(c, f);
+  int rc = DISPATCH(c, get_conserved_t)(c, dev);
+  if (rc) return rc;
+  rc = cuda_call(c, cudaEventRecord(c->ev_out_ready, c->stream));
+  if (!rc) rc = cuda_call(c, cudaStreamWaitEvent(c->d2h_stream, c->ev_out_ready, 0));
+  size_t bytes = (size_t)c->L.nx * c->L.ny * c->L.nz * c->elem;
+  for (int f = 0; f < 5 && !rc; ++f)
+    rc = cuda_call(c, cudaMemcpyAsync(host[f], dev[f], bytes, cudaMemcpyDeviceToHost, c->d2h_stream));
+  if (!rc) rc = cuda_call(c, cudaEventRecord(c->ev_out_done, c->d2h_stream));
+  c->out_pending = true;
+  return rc;
+}
+
 int cspt_set_conserved(cspt_ctx* c, const void* rho, const void* mx, const void* my, const void* mz, const void* E) {
   if (!c || !rho || !mx || !my || !mz || !E) return CSPT_EINVAL;
   if (!c->has_state) return CSPT_ESTATE;
@@ -961,7 +1030,10 @@ int cspt_cuda_error(const cspt_ctx* c) { return c ? c->cuda_error : 0; }
 int cspt_sync(cspt_ctx* c) {
   if (!c) return CSPT_EINVAL;
   if (c->cuda_error) return CSPT_ECUDA;
-  return cuda_call(c, cudaStreamSynchronize(c->stream));
+  int rc = cuda_call(c, cudaStreamSynchronize(c->stream));
+  if (!rc && c->h2d_stream) rc = cuda_call(c, cudaStreamSynchronize(c->h2d_stream));
+  if (!rc && c->d2h_stream) rc = cuda_call(c, cudaStreamSynchronize(c->d2h_stream));
+  return rc;
 }
 
 const char* cspt_strerror(int code) {

@@ -130,6 +130,11 @@ struct cspt_ctx {
   int riemann;              // CSPT_RIEMANN_*: flux at the faces of the Euler stage
   int euler_variant;        // 0: one thread per cell with shared-memory flux exchange, 1: rows + helper warp
   int corr_variant;         // 0: 26-neighbour corrector, 1: pair-symmetric strips with shared x pairs (warp shuffles)
+  // asynchronous host entry points (cspt_*_host_async): copy streams of their own, so that the device-to-host copy of
+  // one result and the host-to-device copy of the next input use both directions of the link at once
+  cudaStream_t h2d_stream, d2h_stream;
+  cudaEvent_t ev_in_free, ev_in_ready, ev_out_ready, ev_out_done;
+  bool out_pending;                 // a device-to-host copy may still read its staging slots (U~ / xi slots)
   // CUDA graphs of two consecutive cspt_step_cfl steps (cspt_run_cfl), one per parity of `cur` at entry
   cudaGraphExec_t graph[2];
   cudaStream_t gstream;             // capture / replay stream of a ctx that lives on the legacy default stream

@@ -424,6 +424,37 @@ def test_host_entry_points_roundtrip(cspt, oracle_mod):
         assert torch.equal(x.cpu(), y)
 
 
+def test_async_host_entry_points_match_the_blocking_ones(cspt, oracle_mod):
+    """cspt_set_state_host_async / cspt_get_conserved_host_async (copy streams of their own) against the blocking calls,
+    over three back-to-back states whose copies overlap: same bits, and a step in between waits for the staged result."""
+    import torch
+    ws = [wl.random_smooth(40, 24, 20, seed=s0) for s0 in (3, 4, 5)]
+    w = ws[0]
+    fields = [[torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in x.fields()] for x in ws]
+    ref = []
+    s = make_solver(cspt, w)
+    for f in fields:
+        out = [torch.empty((w.nz, w.ny, w.nx), dtype=torch.float64).pin_memory() for _ in range(5)]
+        s.set_state_host(*f)
+        s.step_cfl(w.cfl)
+        s.step_cfl(w.cfl)
+        s.get_conserved_host(out)
+        ref.append([t.clone() for t in out])
+    s.close()
+    s = make_solver(cspt, w)
+    outs = [[torch.empty((w.nz, w.ny, w.nx), dtype=torch.float64).pin_memory() for _ in range(5)] for _ in fields]
+    for f, out in zip(fields, outs):
+        s.set_state_host_async(*f)
+        s.step_cfl(w.cfl)
+        s.step_cfl(w.cfl)
+        s.get_conserved_host_async(out)
+    s.sync()
+    for a, b in zip(ref, outs):
+        for x, y in zip(a, b):
+            assert torch.equal(x, y)
+    s.close()
+
+
 def test_explicit_stream_and_two_solvers_alive(cspt, oracle_mod):
     """The ctx works on the stream it was given (not only torch's current stream), and two solvers of different
     precision and size can be interleaved on their own streams."""
