@@ -47,7 +47,8 @@ enum { CSPT_LIMITER_MINMOD = 0, CSPT_LIMITER_VANLEER = 1 };
 enum { CSPT_RIEMANN_HLL = 0, CSPT_RIEMANN_LF = 1, CSPT_RIEMANN_HLLC = 2 };
 /* smoothing kernel W of Eq. (7) (PAPER.md:68 leaves it open, :133): the cubic spline is the default (reading G5) */
 enum { CSPT_KERNEL_CUBIC_SPLINE = 0, CSPT_KERNEL_POLY5 = 1 };
-enum { CSPT_OK = 0, CSPT_EINVAL = -1, CSPT_ENOMEM = -2, CSPT_ECUDA = -3, CSPT_ESTATE = -4 };
+enum { CSPT_OK = 0, CSPT_EINVAL = -1, CSPT_ENOMEM = -2, CSPT_ECUDA = -3, CSPT_ESTATE = -4,
+       CSPT_ELIMIT = -5 /* a size beyond the fixed capacity of cspt_cfl_dt_noalloc's built-in scratch */ };
 
 /* Bytes of device workspace cspt_create needs for this grid (0 if the arguments
  * are invalid).  The caller allocates it (256-byte aligned), e.g. with torch. */
@@ -195,6 +196,38 @@ int cspt_halo_put(cspt_ctx*, int face, int what, const void* device_buf);
 int cspt_finish_state(cspt_ctx*);
 int cspt_fill_ghosts(cspt_ctx*);
 int cspt_step_filled(cspt_ctx*, double dt);
+/* ---- CFL time step without a ctx, a workspace or any allocation ------------------------------------------------
+ * For callers that cannot allocate device memory.  cspt_compute_dt needs a ctx, and a ctx needs a workspace of 28
+ * padded fields that someone must allocate.  That is impossible for a host code that gave all of HBM to its own arena
+ * at start-up, unwelcome inside a time loop (cudaMalloc / cudaFree stall the whole device), and not an option for an
+ * in-situ monitor or a coupled solver that is merely handed device pointers to the conserved fields and has to answer
+ * with a common time step.  This call serves them: it computes the same CFL time step (reading G15; the paper is
+ * silent) from five DENSE device arrays rho, rho u, rho v, rho w, E of ncells elements each (any order: the result
+ * does not depend on it; no ghost cells), in the arithmetic of cspt_compute_dt, bit for bit:
+ *     *dt_device_out = (cfl*h) / max_cells(c + max(|u|,|v|,|w|)),  c = sqrt(gamma p / rho),  cells with rho <= 1e-12
+ *     skipped (reading G9);  +inf if ncells = 0 or every cell is vacuum.
+ * dtype: CSPT_F64 (double arrays, double result) or CSPT_F32 (float arrays, float result; h, gamma, cfl rounded to
+ * float once).  dt_device_out: ONE element of that type in device memory, the caller's.  cuda_stream: a cudaStream_t
+ * of the current device (NULL = default stream).  Two kernels are enqueued on it; the call does not sync, and it calls
+ * no cudaMalloc, cudaFree or other allocating routine.
+ *
+ * Its scratch (one maximum per 4096 cells) is a fixed array inside the library's device code: 65536 slots = 512 KiB
+ * on every GPU that loads libcspt.so, held until the process exits.  Hence the limit
+ *     ncells <= CSPT_NOALLOC_MAX_CELLS = 65536 * 4096 = 268 435 456   (512^3 fits, 1024^3 does not);
+ * beyond it the call does nothing and returns CSPT_ELIMIT ("beyond the fixed capacity of the built-in scratch").
+ * All calls on one device share that array, whatever their stream, and each finds the previous call's values in
+ * it.  Nothing in it has to be zero at entry (each call reads back only the slots it has just written), but two calls
+ * whose kernels may overlap on the GPU -- different streams without an event between them, or several host threads --
+ * race on it and may both return a wrong time step: keep calls on one device ordered.
+ * The FIRST call on each device looks up the device address of the array (cudaGetSymbolAddress, with that device
+ * current) and keeps it; make that first call with the right device current and before any stream capture begins.
+ * EINVAL: unknown dtype, ncells < 0, a null array with ncells > 0, null dt_device_out, h <= 0, gamma <= 1, cfl <= 0
+ * or not finite.  ELIMIT: ncells too large (or a device ordinal >= 64).  ECUDA: the address lookup or a launch failed
+ * (cudaGetLastError tells which error). */
+#define CSPT_NOALLOC_MAX_CELLS 268435456LL
+long long cspt_noalloc_max_cells(void);      /* the same number, for bindings that cannot read macros */
+int cspt_cfl_dt_noalloc(int dtype, long long ncells, const void* rho, const void* mx, const void* my, const void* mz,
+                        const void* E, double gamma, double h, double cfl, void* dt_device_out, void* cuda_stream);
 /* The cudaError_t value behind a CSPT_ECUDA status of this ctx (0 if none). */
 int cspt_cuda_error(const cspt_ctx*);
 /* Waits for the ctx's stream and for the copy streams of the *_host_async calls. */

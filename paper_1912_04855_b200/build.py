@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcspt.so")
-SOURCES = ["cspt_api.cu"]
+SOURCES = ["cspt_api.cu", "cspt_noalloc.cu"]
 HEADERS = ["cspt_common.cuh", "cspt_kernels.cuh", "cspt_tma.cuh", "cspt_euler.cuh", "cspt_lagrange.cuh", "cspt_corrector.cuh", "cspt_euler2.cuh"]
 
 NVCC_FLAGS = [

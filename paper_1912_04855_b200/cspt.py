@@ -15,7 +15,7 @@ HALO_U, HALO_PSI = 0, 1
 LIMITER_MINMOD, LIMITER_VANLEER = 0, 1
 KERNEL_CUBIC_SPLINE, KERNEL_POLY5 = 0, 1
 RIEMANN_HLL, RIEMANN_LF, RIEMANN_HLLC = 0, 1, 2
-OK, EINVAL, ENOMEM, ECUDA, ESTATE = 0, -1, -2, -3, -4
+OK, EINVAL, ENOMEM, ECUDA, ESTATE, ELIMIT = 0, -1, -2, -3, -4, -5
 
 # every symbol include/cspt.h declares: (name, restype, argtypes)
 _vp, _ci, _cd, _sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
@@ -51,6 +51,8 @@ SYMBOLS = [
     ("cspt_finish_state", _ci, [_vp]),
     ("cspt_fill_ghosts", _ci, [_vp]),
     ("cspt_step_filled", _ci, [_vp, _cd]),
+    ("cspt_noalloc_max_cells", ctypes.c_longlong, []),
+    ("cspt_cfl_dt_noalloc", _ci, [_ci, ctypes.c_longlong, _vp, _vp, _vp, _vp, _vp, _cd, _cd, _cd, _vp, _vp]),
     ("cspt_cuda_error", _ci, [_vp]),
     ("cspt_sync", _ci, [_vp]),
     ("cspt_destroy", None, [_vp]),
@@ -90,6 +92,33 @@ def _check(code, where):
 
 def _dptr(t):
     return ctypes.c_void_p(t.data_ptr())
+
+
+def noalloc_max_cells():
+    """Largest ncells cspt_cfl_dt_noalloc accepts (its scratch is a fixed array inside the library)."""
+    return int(lib().cspt_noalloc_max_cells())
+
+
+def cfl_dt_noalloc(rho, mx, my, mz, E, gamma, h, cfl, out, stream=None):
+    """cspt_cfl_dt_noalloc: the CFL time step of five dense, contiguous CUDA tensors of conserved variables, written
+    into the caller's one-element CUDA tensor `out` of the same dtype (float64 or float32).  For callers that hold the
+    fields but cannot allocate a ctx workspace (all memory in the application's own pool, no cudaMalloc allowed in the
+    time loop, plug-in monitors that only receive pointers): neither this binding nor the library allocates anything,
+    which is why `out` is an argument and not a return value.  Enqueues on `stream` (default: torch's current stream)
+    and does not sync; calls on one device must not overlap (they share the library's built-in scratch).  Sizes
+    above noalloc_max_cells() raise CsptError with code ELIMIT."""
+    import torch
+    ts = (rho, mx, my, mz, E)
+    dt = ts[0].dtype
+    assert dt in (torch.float64, torch.float32)
+    assert all(t.is_cuda and t.dtype == dt and t.is_contiguous() and t.numel() == ts[0].numel() for t in ts)
+    assert out.is_cuda and out.dtype == dt and out.numel() == 1 and out.device == ts[0].device
+    assert torch.cuda.current_device() == ts[0].device.index, "make the tensors' device current first"
+    st = stream if stream is not None else torch.cuda.current_stream()
+    _check(lib().cspt_cfl_dt_noalloc(F64 if dt == torch.float64 else F32, ts[0].numel(), *[_dptr(t) for t in ts],
+                                     float(gamma), float(h), float(cfl), _dptr(out), ctypes.c_void_p(st.cuda_stream)),
+           "cspt_cfl_dt_noalloc")
+    return out
 
 
 class Solver:

@@ -1043,6 +1043,7 @@ const char* cspt_strerror(int code) {
     case CSPT_ENOMEM: return "out of host memory";
     case CSPT_ECUDA: return "CUDA error (sticky until destroy)";
     case CSPT_ESTATE: return "no state set";
+    case CSPT_ELIMIT: return "size beyond the fixed capacity of the built-in scratch (cspt_cfl_dt_noalloc)";
     default: return "unknown status";
   }
 }
