@@ -20,9 +20,11 @@
 // form; brute-force all-pairs evaluation of Eq. (7); closed-form lattice
 // weights; free fall in a linear potential; the ghost rules of every boundary
 // kind on non-uniform states, the pressure floor, the LF / HLL / HLLC face
-// fluxes against the textbook solvers; the paper's printed order 1.94 for the
-// linear transfer of a smooth wave on N = 400, 800, 1600 (reading
-// G23 (i)).  Parity that stays UNPINNED: agreement with the authors' own code
+// fluxes against the textbook solvers; second order for the linear transfer of
+// a smooth wave on N = 400, 800, 1600 (reading G23 (i)); the
+// ballistic particle offsets of Eq. (5), (6) in uniform free fall and the
+// vacuum threshold of reading G9 (tests/test_oracle_round3_pins.py).
+// Parity that stays UNPINNED: agreement with the authors' own code
 // (kernel, limiter, Riemann solver, CFL rule and boundary rules are readings,
 // DESIGN.md section 3), second order on a nonlinear simple wave (reading
 // G23 (ii): measured first order) and the Fig. 1 shock position (parameters
@@ -647,6 +649,18 @@ void orc_get_padded(void* vh, int c, void* out) {
   Handle* hd = (Handle*)vh;
   if (c < 0 || c > 4) return;
 #define BODY { o->fill_ghosts_U(false); memcpy(out, o->U[c].data(), o->ncell_pad * sizeof(T)); }
+  DISPATCH(hd, BODY, BODY);
+#undef BODY
+}
+
+// Particle offsets of the LAST step (read-only test hook): which = 0: xi* of Eq. (5), valid on
+// interior(+)2; which = 1: xi^{n+1} of Eq. (6), valid on interior(+)1; component d = 0..2; padded
+// (nz+6, ny+6, nx+6) array, x fastest.  Lets a test check the kinematics of Eq. (5), (6) directly: they are Heun's
+// rule for dr/dt = u, which integrates a constant acceleration exactly.
+void orc_get_offsets(void* vh, int which, int d, void* out) {
+  Handle* hd = (Handle*)vh;
+  if (d < 0 || d > 2 || which < 0 || which > 1) return;
+#define BODY { memcpy(out, (which ? o->xi[d] : o->xis[d]).data(), o->ncell_pad * sizeof(T)); }
   DISPATCH(hd, BODY, BODY);
 #undef BODY
 }

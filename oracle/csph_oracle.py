@@ -76,6 +76,8 @@ def _load():
     lib.orc_eval_Q.restype = None
     lib.orc_get_padded.argtypes = [vp, ci, vp]
     lib.orc_get_padded.restype = None
+    lib.orc_get_offsets.argtypes = [vp, ci, ci, vp]
+    lib.orc_get_offsets.restype = None
     lib.orc_lattice_constants.argtypes = [vp, ctypes.POINTER(cd)]
     lib.orc_lattice_constants.restype = None
     _lib = lib
@@ -184,6 +186,13 @@ class Oracle:
         shape (nz+6, ny+6, nx+6)."""
         out = np.empty((self.nz + 6, self.ny + 6, self.nx + 6), dtype=self.np_dtype)
         _load().orc_get_padded(self._h, int(c), _ptr(out))
+        return out
+
+    def get_offsets(self, which, d):
+        """Component d of the particle offsets of the last step, padded (nz+6, ny+6, nx+6): which = 0: xi* of
+        Eq. (5), valid on interior(+)2; which = 1: xi^{n+1} of Eq. (6), valid on interior(+)1."""
+        out = np.empty((self.nz + 6, self.ny + 6, self.nx + 6), dtype=self.np_dtype)
+        _load().orc_get_offsets(self._h, int(which), int(d), _ptr(out))
         return out
 
     def lattice_constants(self):

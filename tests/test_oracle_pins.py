@@ -551,8 +551,10 @@ def test_simple_wave_order_is_reported_as_measured(oracle_mod):
 def test_linear_transfer_of_a_smooth_wave_at_the_papers_resolutions(oracle_mod):
     """'linear transfer of smooth Riemann wave ... N = 400, 800, 1600, 3200, 6400 ... approximation order
     of about 1.94; order of convergence is 2.04'.  Read as LINEAR transport (the profile is carried by a uniform flow,
-    exact solution = translation; reading G23 (i)) the oracle reproduces the printed 1.94 on the paper's first three
-    grids with the default minmod limiter (measured 1.93, 1.95), and 2.09 with van Leer's limiter."""
+    exact solution = translation; reading G23 (i)) the oracle is second order on the paper's first three grids with the
+    default minmod limiter (measured 1.93, 1.95) and with van Leer's limiter (2.09).  The paper gives no set-up
+    (t_end = 0.125 and the amplitude 0.2 are this test's), so the closeness to the printed 1.94 is NOT a pin of the
+    paper's number: this is a second-order check for div u = 0 transport, nothing more."""
     t_end, u0 = 0.125, 1.0
     found = {}
     for lim, grids in ((0, (400, 800, 1600)), (1, (400, 800))):
@@ -569,5 +571,5 @@ def test_linear_transfer_of_a_smooth_wave_at_the_papers_resolutions(oracle_mod):
             errs.append(float(np.mean(np.abs(o.get_state()[0].ravel() - exact))))
         found[lim] = [math.log2(errs[i] / errs[i + 1]) for i in range(len(grids) - 1)]
     print("linear transfer orders (minmod, van Leer):", found)
-    assert all(abs(q - 1.94) < 0.04 for q in found[0]), found          # the paper's printed 1.94
+    assert all(q > 1.85 for q in found[0]), found                      # second order (the paper prints 1.94)
     assert all(1.95 < q < 2.15 for q in found[1]), found
