@@ -384,10 +384,10 @@ def run_configs(cspt, peak, headline):
 
 # algorithmic work of the corrector's neighbour sum, per neighbour [3 sub, 3 FMA for r^2, 1 rsqrt,
 # 5 for the spline, 1 mul, 3 FMA, 3 add, 3 FMA, 1 FMA] = 23 FP instructions (FMA counted once), 26 neighbours,
-# + about 40 for Eq. (6); in flops (FMA = 2): 36 per neighbour + 60.  The implementation evaluates pairs once and
+# + about 40 for Eq. (6); in flops (FMA = 2): 3 + 6 + 1 + 5 + 1 + 6 + 3 + 6 + 2 = 33 per neighbour, + 60.  The implementation evaluates pairs once and
 # executes FEWER instructions than this list; the roofline fraction is quoted on the list, not on what was executed.
 ALGO_INSTR = {"corrector": 26 * 23 + 40}
-ALGO_FLOPS = {"corrector": 26 * 36 + 60}
+ALGO_FLOPS = {"corrector": 26 * 33 + 60}
 
 
 def run_cspt(args):
@@ -430,9 +430,21 @@ def run_cspt(args):
         s.step_cfl(w.cfl)
     s.run_cfl(w.cfl, 2)                  # graph capture outside the timed region
     barrier()
-    fma_rate = s.probe_fma_rate()        # roofline denominator, measured on this box in this run
-    issue_probe = {str(k): s.probe_fma_rate(k) for k in (1, 2, 4, 8)}
-    fma_rate3 = s.probe_fma_rate(-1)     # FMAs with three distinct register operands (register-file bound in fp64)
+    # FMA probe of the plain FP pipe, run for >= 80 ms with the SM clock sampled DURING it, so that its rate can be
+    # quoted per clock and SM; it is a CHECK beside the architectural peak the roofline is quoted on, not the peak
+    sm_count = s.sm_count()
+    probe_sampler = ClockSampler(local)
+    probe_sampler.start()
+    try:
+        fma_rate = s.probe_fma_rate(0, min_ms=80.0)
+        probe_err = None
+    except cspt.CsptError as e:          # never lose the bench line to the probe
+        fma_rate, probe_err = None, repr(e)
+    probe_clocks = probe_sampler.stop()
+    issue_probe, fma_rate3 = {}, None
+    if fma_rate:
+        issue_probe = {str(k): s.probe_fma_rate(k, min_ms=10.0) for k in (1, 2, 4, 8)}
+        fma_rate3 = s.probe_fma_rate(-1, min_ms=10.0)   # FMAs with three distinct register operands (register-file bound in fp64)
     barrier()
 
     # ---- timed region: exactly K steps (cspt_run_cfl), device time from CUDA events on the launching stream,
@@ -452,12 +464,15 @@ def run_cspt(args):
     value = job_value(w.cells, args.steps, world, tmax)
 
     # ---- the same K steps once more with an event pair around every launch: per-kernel times for the roofline
+    prof_sampler = ClockSampler(local)
+    prof_sampler.start()
     s.profile_enable(True)
     for _ in range(args.steps):
         s.step_cfl(w.cfl)
     prof = s.profile_read()
     s.profile_enable(False)
     barrier()
+    prof_clocks = prof_sampler.stop()
 
     # the state must still be sane (a blown-up run would time NaN arithmetic)
     rho = s.get_conserved()[0]
@@ -518,27 +533,41 @@ def run_cspt(args):
            "algorithmic_bytes_per_launch": dom_bytes}
     share = (prof[dom][0] / prof_steps) / prof_step_ms
     if dom in ALGO_FLOPS and args.kernel == "cubic":
-        # the corrector is bound by the plain FP64 / FP32 pipe.  Denominator: the FMA rate
-        # cspt_probe_fma_rate measured in THIS run just before the timed region (thread-level FMA/s; an FP instruction
-        # of any kind occupies a lane of that pipe for one slot, so it is also the instruction rate).
-        apeak = 2.0 * fma_rate / 1e12
-        aach = ALGO_FLOPS[dom] * w.cells / (dom_ms * 1e-3) / 1e12
-        roofline = {"bound": "alu", "kernel": dom, "achieved": aach, "peak": apeak, "unit": "TFLOP/s",
-                    "frac": aach / apeak, "frac_is": "flop fraction (FMA = 2 flop) of the measured FMA peak",
-                    "instr_frac": ALGO_INSTR[dom] * w.cells / (dom_ms * 1e-3) / fma_rate,
-                    "instr_frac_is": "SURVEY 8(d) instruction list (%d FP instructions per cell, FMA counted once) over "
-                                     "the measured instruction rate of the pipe" % ALGO_INSTR[dom],
+        # The corrector is bound by the plain FP64 / FP32 pipe.  Roofline as SURVEY 8(d) states it:
+        # the survey's instruction list per cell (FMA counted once) over the ARCHITECTURAL rate of that pipe,
+        # lanes x SMs x the maximum SM clock (64 FP64 / 128 FP32 lanes per SM, B200_PROFILING.md); an FP instruction
+        # of any kind holds a lane for one slot.  Beside it: the same over the clock NVML sampled while the kernel
+        # times were taken, the flop version (FMA = 2), and the in-run FMA probe with ITS sampled clock as a check.
+        lanes = 64 if w.dtype == "f64" else 128
+        max_mhz = clocks.get("sm_max_mhz") or 1965
+        peak_i = lanes * sm_count * max_mhz * 1e6 / 1e12                 # T FP instructions / s
+        ach_i = ALGO_INSTR[dom] * w.cells / (dom_ms * 1e-3) / 1e12
+        ach_f = ALGO_FLOPS[dom] * w.cells / (dom_ms * 1e-3) / 1e12
+        run_mhz = prof_clocks.get("sm_mhz") or clocks.get("sm_mhz")
+        probe = None
+        if fma_rate:
+            pm = probe_clocks.get("sm_mhz")
+            probe = {"fma_per_second": fma_rate, "sm_mhz_during_probe": pm, "probe_clocks": probe_clocks,
+                     "fma_per_clock_per_sm": fma_rate / sm_count / (pm * 1e6) if pm else None,
+                     "lanes_per_sm": lanes, "instr_frac_of_probe": ach_i * 1e12 / fma_rate,
+                     "fma_per_second_three_register_operands": fma_rate3,
+                     "fma_per_second_with_other_instructions": issue_probe,
+                     "issue_note": "FMA rate with 1 / 2 / 4 / 8 independent integer instructions behind every FMA: cycles "
+                                   "per FMA and SMSP ~ max(pipe, 1.1 * (1 + others)), pipe = 2 in fp64 and 1 in fp32 "
+                                   "(DESIGN.md section 7, profiles/r2_issue_model.md)"}
+        roofline = {"bound": "alu", "kernel": dom, "achieved": ach_i, "peak": peak_i, "unit": "T FP instr/s",
+                    "frac": ach_i / peak_i,
+                    "frac_is": "SURVEY 8(d) instruction list of the corrector (%d FP instructions per cell, FMA counted once) "
+                               "x cells / kernel time, over %d lanes x %d SMs x %d MHz (maximum SM clock)"
+                               % (ALGO_INSTR[dom], lanes, sm_count, max_mhz),
+                    "peak_source": "architectural: lanes x SMs x sm_max_mhz (B200_PROFILING.md unit counts; NVML max clock)",
+                    "frac_at_sampled_clock": ach_i / (lanes * sm_count * run_mhz * 1e6 / 1e12) if run_mhz else None,
+                    "sampled_clock_mhz": run_mhz, "clocks_during_kernel_timing": prof_clocks,
+                    "flops": {"achieved": ach_f, "peak": 2.0 * peak_i, "unit": "TFLOP/s", "frac": ach_f / (2.0 * peak_i),
+                              "per_cell": ALGO_FLOPS[dom],
+                              "note": "33 flop per neighbour (the survey's list, FMA = 2) x 26 + 60 for Eq. (6)"},
                     "traffic": traffic, "traffic_source": traffic_src, "ncu": ncu_stored,
-                    "peak_source": "measured in this run: cspt_probe_fma_rate, %.1f %s FMA per clock per SM at %d MHz"
-                                   % (fma_rate / 148 / ((clocks.get("sm_max_mhz") or 1965) * 1e6), w.dtype,
-                                      clocks.get("sm_max_mhz") or 1965),
-                    "fma_per_second": fma_rate,
-                    "fma_per_second_three_register_operands": fma_rate3,
-                    "fma_per_second_with_other_instructions": issue_probe,
-                    "issue_note": "FMA rate with 1 / 2 / 4 / 8 independent integer instructions behind every FMA: cycles per "
-                                  "FMA and SMSP ~ max(pipe, 1.1 * (1 + others)), pipe = 2 in fp64 and 1 in fp32 "
-                                  "(DESIGN.md section 7, profiles/r2_issue_model.md)",
-                    "algorithmic_flops_per_cell": ALGO_FLOPS[dom],
+                    "probe": probe, "probe_error": probe_err,
                     "algorithmic_instr_per_cell": ALGO_INSTR[dom], "kernel_ms": dom_ms, "share_of_step": share,
                     "hbm": hbm}
     else:
@@ -550,11 +579,11 @@ def run_cspt(args):
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": step_ms, "kernels": kern, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": w.dtype, "data": "synthetic",
         "config": dict(config_of(w, world), limiter=args.limiter, kernel=args.kernel, riemann=args.riemann,
                        api="cspt_run_cfl"),
-        "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "kernels": kern,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
         "kernels_note": "per-kernel times from a second pass of the same K steps with an event pair around every launch "
                         "(%.3f ms per step in that pass, %d steps recorded)" % (prof_step_ms, prof_steps),
         "roofline": roofline, "step_hbm": step_hbm,

@@ -110,7 +110,8 @@ int cspt_set_limiter(cspt_ctx*, int limiter);
  *   CSPT_RIEMANN_HLLC contact speed S* = (rho^L u^L + rho^R u^R)/(rho^L + rho^R) between converging streams, star
  *                     state of Toro's HLLC with p = 0; equal to HLL at every other face.
  * Takes effect from the next step.  Host-side only (LF / HLLC move a CSPT_F32 ctx to the kernel layout that
- * exchanges face states).  EINVAL: null ctx or unknown solver. */
+ * exchanges face states; selecting HLL again moves it back, so a ctx set to HLL always runs the same kernels whatever
+ * was selected before).  EINVAL: null ctx or unknown solver. */
 int cspt_set_riemann(cspt_ctx*, int riemann);
 
 /* One full step U^n -> U^{n+1} with time step dt (Eq. (4)-(8)): ghost fill,
@@ -148,6 +149,7 @@ int cspt_set_conserved(cspt_ctx*, const void* rho, const void* mx, const void* m
 /* mask[i] = 1 where rho <= rho_vac = 1e-12 (reading G9), else 0.  Device pointer. */
 int cspt_get_vacuum_mask(cspt_ctx*, unsigned char* mask);
 
+/* ---- DIAGNOSTICS (measurement aids of bench.py and the tests; not part of the method) --------------------------- */
 /* Number of kernel launches issued by this ctx so far (for bench.py's gpu_launches). */
 long long cspt_launch_count(const cspt_ctx*);
 /* Per-kernel device timing.  While enabled, every kernel the ctx launches is bracketed
@@ -169,6 +171,18 @@ int cspt_profile_read(cspt_ctx*, int kid, double* total_ms, long long* launches)
  * (x = y * z + x): in fp64 each is a register pair and the register file delivers two pairs per cycle, so these issue
  * every 3 cycles.  EINVAL: other_per_fma not one of -1, 0, 1, 2, 4, 8. */
 int cspt_probe_fma_rate(cspt_ctx*, int other_per_fma, double* fma_per_second);
+/* The same probe (one launch lasts about 3 ms), repeated back to back until the timed region lasts at least min_ms
+ * (0 <= min_ms <= 10000): long enough for the GPU to settle into the power state a long step runs in and for an NVML
+ * clock sampler to see it, so that the rate can be quoted per clock.  The launch fills every SM the device has
+ * (cspt_sm_count) on any grid size.  EINVAL as above, or min_ms out of range. */
+int cspt_probe_fma_rate_ms(cspt_ctx*, int other_per_fma, double min_ms, double* fma_per_second);
+/* Multiprocessors of the device the ctx was created on (0 for a null ctx). */
+int cspt_sm_count(const cspt_ctx*);
+/* The fp32 Euler stage exists with and without its gas-vacuum shortcuts; a hint from cspt_set_state picks one, and both
+ * give the same bits.  force = 0 / 1 pins the variant without / with the shortcuts (the test of that equality),
+ * -1 follows the hint again.  Host-side only.  EINVAL: null ctx, force not in {-1, 0, 1}. */
+int cspt_debug_force_vacuum_variant(cspt_ctx*, int force);
+/* ---- end of diagnostics ------------------------------------------------------------------------------------------ */
 /* ---- z-slab decomposition over several GPUs ("the computational domain is divided between GPUs",
  * :123).  One ctx per slab of nz_local planes; a z face that borders another slab has
  * kind CSPT_BC_EXTERNAL.  The dependence of one step reaches 3 cells (reading G16), and every intermediate
@@ -189,7 +203,9 @@ int cspt_probe_fma_rate(cspt_ctx*, int other_per_fma, double* fma_per_second);
  * cspt_halo_put: writes such a message into the 3 ghost planes of `face`, which must be EXTERNAL (else EINVAL).
  * cspt_finish_state: forms f = -D[psi] (S2) once the psi ghost planes are in place; ESTATE if no cspt_set_state is
  *   pending.  cspt_fill_ghosts: S0 on every face that is not EXTERNAL.  cspt_step_filled: S1..S9 with the given dt on a
- *   state whose ghost layers are complete.  All enqueue on the ctx's stream and do not sync. */
+ *   state whose ghost layers are complete: ESTATE unless, since the state last changed (a step, cspt_set_state,
+ *   cspt_set_conserved), cspt_fill_ghosts has run and every EXTERNAL face has received its cspt_halo_put(CSPT_HALO_U).
+ *   All enqueue on the ctx's stream and do not sync. */
 int cspt_halo_elems(const cspt_ctx*, int what, long long* elems);
 int cspt_halo_get(cspt_ctx*, int face, int what, void* device_buf);
 int cspt_halo_put(cspt_ctx*, int face, int what, const void* device_buf);

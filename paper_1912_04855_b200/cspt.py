@@ -45,6 +45,9 @@ SYMBOLS = [
     ("cspt_profile_kernel_name", ctypes.c_char_p, [_ci]),
     ("cspt_profile_read", _ci, [_vp, _ci, _pd, ctypes.POINTER(ctypes.c_longlong)]),
     ("cspt_probe_fma_rate", _ci, [_vp, _ci, _pd]),
+    ("cspt_probe_fma_rate_ms", _ci, [_vp, _ci, _cd, _pd]),
+    ("cspt_sm_count", _ci, [_vp]),
+    ("cspt_debug_force_vacuum_variant", _ci, [_vp, _ci]),
     ("cspt_halo_elems", _ci, [_vp, _ci, ctypes.POINTER(ctypes.c_longlong)]),
     ("cspt_halo_get", _ci, [_vp, _ci, _ci, _vp]),
     ("cspt_halo_put", _ci, [_vp, _ci, _ci, _vp]),
@@ -287,12 +290,23 @@ class Solver:
                 out[L.cspt_profile_kernel_name(kid).decode()] = (ms.value, int(n.value))
         return out
 
-    def probe_fma_rate(self, other_per_fma=0):
+    def probe_fma_rate(self, other_per_fma=0, min_ms=0.0):
         """Measured FMA rate of the plain FP pipe in the solver's precision (thread-level FMAs per second), alone or
-        with 2 / 4 / 8 independent integer instructions interleaved per FMA."""
+        with 2 / 4 / 8 independent integer instructions interleaved per FMA; min_ms > 0 repeats the probe until it has
+        run that long (cspt_probe_fma_rate_ms)."""
         out = ctypes.c_double()
-        _check(lib().cspt_probe_fma_rate(self._h, int(other_per_fma), ctypes.byref(out)), "cspt_probe_fma_rate")
+        if min_ms:
+            _check(lib().cspt_probe_fma_rate_ms(self._h, int(other_per_fma), float(min_ms), ctypes.byref(out)),
+                   "cspt_probe_fma_rate_ms")
+        else:
+            _check(lib().cspt_probe_fma_rate(self._h, int(other_per_fma), ctypes.byref(out)), "cspt_probe_fma_rate")
         return out.value
+
+    def debug_force_vacuum_variant(self, force):
+        _check(lib().cspt_debug_force_vacuum_variant(self._h, int(force)), "cspt_debug_force_vacuum_variant")
+
+    def sm_count(self):
+        return int(lib().cspt_sm_count(self._h))
 
     # -- z-slab decomposition (include/cspt.h: CSPT_BC_EXTERNAL) ---------------------------------------
     def halo_elems(self, what=HALO_U):

@@ -121,6 +121,9 @@ void fill_ghosts(cspt_ctx* c, T* F, int nfields, int mode) {
   }
 }
 
+// the ghost layers of the current U (boundary rules and slab halos) no longer belong to it
+inline void stale_ghosts(cspt_ctx* c) { c->ghosts_current = false; c->halo_current[0] = c->halo_current[1] = false; }
+
 inline bool has_external(const cspt_ctx* c) { return c->bc[4] == CSPT_BC_EXTERNAL || c->bc[5] == CSPT_BC_EXTERNAL; }
 
 // S2: f = -D[psi] on interior(+)2 from the padded psi (all ghost layers filled)
@@ -162,6 +165,7 @@ int halo_copy_t(cspt_ctx* c, int face, int what, void* buf, bool put) {
 template <class T>
 int fill_ghosts_t(cspt_ctx* c) {
   fill_ghosts<T>(c, field<T>(c, c->cur ? S_U1 : S_U0), 5, 0);
+  c->ghosts_current = true;
   return check(c);
 }
 
@@ -186,6 +190,7 @@ int set_state_t(cspt_ctx* c, const void* rho, const void* u, const void* v, cons
   c->smax_valid = false;
   c->has_state = false;
   c->force_pending = true;
+  stale_ghosts(c);
   // a slab (EXTERNAL z faces) needs the psi ghost planes of its neighbours before f = -D[psi] can be formed there:
   // cspt_halo_get/put(CSPT_HALO_PSI), then cspt_finish_state
   if (has_external(c)) return check(c);
@@ -201,6 +206,7 @@ int set_conserved_t(cspt_ctx* c, const void* const in[5]) {
   c->vac_pending = false;        // the new state was not looked at: keep the shortcuts on
   c->vac_hint = 1;
   c->smax_valid = false;
+  stale_ghosts(c);
   return check(c);
 }
 
@@ -338,9 +344,12 @@ bool pair_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
 
 template <class T>
 bool corr_select(cspt_ctx* c, const Params<T>* P, const T* U) {
-  const bool xp = c->bc[0] == CSPT_BC_PERIODIC;
-  if (c->corr_variant == 0) return corr_dispatch<T>(c, P, U);
-  return xp ? pair_variant<T, 8, 4, 2, 1, 1>(c, P, U) : pair_variant<T, 8, 4, 2, 0, 1>(c, P, U);
+  // one layout per precision, each the fastest measured on B200 (profiles/r2_kernels.md); the other is not compiled
+  if constexpr (sizeof(T) == 4) return corr_dispatch<T>(c, P, U);
+  else {
+    const bool xp = c->bc[0] == CSPT_BC_PERIODIC;
+    return xp ? pair_variant<T, 8, 4, 2, 1, 1>(c, P, U) : pair_variant<T, 8, 4, 2, 0, 1>(c, P, U);
+  }
 }
 
 // Euler stage, second layout (cspt_euler2.cuh): TY rows of 32 cells + one helper warp per CTA.
@@ -412,11 +421,17 @@ bool euler_select(cspt_ctx* c, const Params<T>* P, const T* U, T* UN) {
   else return euler2_variant<T, 7, 3, 1>(c, P, U, UN);
 }
 
+// tensor maps and shared-memory attributes of the Euler layout the ctx is on (the cell-per-thread layout exists in
+// fp32 only)
+template <class T>
+bool euler_setup(cspt_ctx* c) {
+  if constexpr (sizeof(T) == 4) { if (c->euler_variant == 0) return euler1_setup<T>(c); }
+  return euler_select<T>(c, nullptr, nullptr, nullptr);
+}
+
 template <class T>
 bool make_maps(cspt_ctx* c) {
-  bool ok = c->euler_variant ? euler_select<T>(c, nullptr, nullptr, nullptr) : euler1_setup<T>(c);
-  ok = ok && corr_select<T>(c, nullptr, nullptr);
-  return ok;
+  return euler_setup<T>(c) && corr_select<T>(c, nullptr, nullptr);
 }
 
 // primitives + HFC/SUL{predictor} over the extended domain interior(+)2: 32 x 4 tiles, inputs through a TMA ring of two
@@ -436,9 +451,7 @@ void launch_predictor(cspt_ctx* c, const Params<T>& P, const T* U) {
     kern<<<grid, PTX * PTY, bytes, c->stream>>>(c->mapPU[c->cur], c->mapPF, P, scalars<T>(c), U, field<T>(c, S_F),
                                                  field<T>(c, S_ST), zc, x0, x1);
   };
-  if (c->pred_stages == 2) launch(k_predictor_stream<T, PTX, PTY, 2>, PredRing<T, PTX, PTY, 2>::BYTES);
-  else if (c->pred_stages == 3) launch(k_predictor_stream<T, PTX, PTY, 3>, PredRing<T, PTX, PTY, 3>::BYTES);
-  else launch(k_predictor_stream<T, PTX, PTY, 0>, 0);
+  launch(k_predictor_stream<T, PTX, PTY, 2>, PredRing<T, PTX, PTY, 2>::BYTES);
   prof_close(c, ps_);
   c->launches++;
 }
@@ -454,9 +467,7 @@ bool predictor_setup(cspt_ctx* c) {
                               R::BXT, PTY + 2, 5);
   ok = ok && make_field_map(&c->mapPF, field<T>(c, S_F), (int)sizeof(T), L.px, L.py, L.pz, L.fstride, 3, R::BXT, PTY, 3);
   ok = ok && cudaFuncSetAttribute(k_predictor_stream<T, PTX, PTY, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                  PredRing<T, PTX, PTY, 2>::BYTES) == cudaSuccess &&
-       cudaFuncSetAttribute(k_predictor_stream<T, PTX, PTY, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                            PredRing<T, PTX, PTY, 3>::BYTES) == cudaSuccess;
+                                  PredRing<T, PTX, PTY, 2>::BYTES) == cudaSuccess;
   return ok;
 }
 
@@ -469,17 +480,22 @@ void launch_corrector(cspt_ctx* c, const Params<T>& P, const T* U) {
 // 1: run the kernel variants with the gas-vacuum shortcuts (the state holds vacuum cells, or nobody has looked yet)
 int vacuum_hint(cspt_ctx* c) {
   if (c->vac_forced >= 0) return c->vac_forced;
-  if (c->vac_pending && cudaEventQuery(c->vac_ev) == cudaSuccess) {
-    c->vac_hint = *(volatile int*)((char*)c->h_pinned + 32) != 0;
-    c->vac_pending = false;
+  if (c->vac_pending) {
+    cudaError_t q = cudaEventQuery(c->vac_ev);
+    if (q == cudaSuccess) {
+      c->vac_hint = *(volatile int*)((char*)c->h_pinned + 32) != 0;
+      c->vac_pending = false;
+    } else if (q == cudaErrorNotReady) {
+      (void)cudaGetLastError();  // "not ready" is not an error of the ctx; anything else stays pending for check()
+    }
   }
-  (void)cudaGetLastError();      // cudaErrorNotReady of the query is not an error of the ctx
   return c->vac_hint;
 }
 
 template <class T>
 void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
-  if (c->euler_variant) { euler_select<T>(c, &P, U, UN); return; }
+  if (sizeof(T) == 8 || c->euler_variant) { euler_select<T>(c, &P, U, UN); return; }
+  if constexpr (sizeof(T) == 4) {
   typedef EulerSmem<T, ETX, EulerTile<T>::TY> S;
   constexpr int ETY = EulerTile<T>::TY;
   const Layout& L = c->L;
@@ -494,6 +510,7 @@ void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
   kern<<<grid, ETX * ETY, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN, &sc->smax_bits, zc);
   prof_close(c, ps_);
   c->launches++;
+  }
 }
 
 // a result on its way to the host (cspt_get_conserved_host_async) is staged in the U~ / xi slots: a step waits for it
@@ -517,6 +534,7 @@ void run_step(cspt_ctx* c, bool fill = true) {
   launch_euler<T>(c, P, U, UN);                                                  // O7, O8 (+O9 epilogue)
   c->cur ^= 1;
   c->smax_valid = true;
+  stale_ghosts(c);               // U^{n+1} has no ghost layers yet
 }
 
 template <class T>
@@ -629,11 +647,13 @@ int run_cfl_t(cspt_ctx* c, double cfl, int nsteps, double* t_out) {
 }
 
 template <class T>
-int probe_fma_t(cspt_ctx* c, int other_per_fma, double* fma_per_second) {
-  // scratch: the star-group slots are dead between steps
+int probe_fma_t(cspt_ctx* c, int other_per_fma, double min_ms, double* fma_per_second) {
+  // scratch: the star-group slots are dead between steps; the kernel's stores are a sink that wraps around it, so
+  // the grid always fills the device (8 CTAs of 128 threads per SM), whatever the size of the ctx's grid
   T* out = field<T>(c, S_ST);
-  const int threads = 128, blocks = 148 * 8, iters = other_per_fma ? 1500 : 4000;
-  if ((long long)threads * blocks > c->L.fstride * 8) return CSPT_EINVAL;
+  const int threads = 128, blocks = c->sm_count * 8, iters = other_per_fma ? 1500 : 4000;
+  long long room = c->L.fstride * 8, want = (long long)threads * blocks;
+  const unsigned cap = (unsigned)(room < want ? room : want);
   auto kern = other_per_fma < 0    ? k_probe_fma<T, -1>
               : other_per_fma == 0 ? k_probe_fma<T, 0>
               : other_per_fma == 1 ? k_probe_fma<T, 1>
@@ -642,18 +662,27 @@ int probe_fma_t(cspt_ctx* c, int other_per_fma, double* fma_per_second) {
                                    : k_probe_fma<T, 8>;
   cudaEvent_t e0, e1;
   if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) { (void)cudaGetLastError(); return CSPT_ECUDA; }
-  kern<<<blocks, threads, 0, c->stream>>>(out, 200, (T)1.0000001, (T)1e-9, 5);          // warm-up
-  cudaEventRecord(e0, c->stream);
-  kern<<<blocks, threads, 0, c->stream>>>(out, iters, (T)1.0000001, (T)1e-9, 5);
-  cudaEventRecord(e1, c->stream);
-  int rc = cuda_call(c, cudaEventSynchronize(e1));
+  kern<<<blocks, threads, 0, c->stream>>>(out, cap, 200, (T)1.0000001, (T)1e-9, 5);          // warm-up
+  c->launches++;
+  // one timed launch first; if the caller wants the probe to last min_ms (so that it runs in the power state a long
+  // step runs in, and a clock sampler sees it), as many launches back to back as that takes are timed as one region
+  int rc = 0, reps = 1;
   float ms = 0;
-  if (!rc) rc = cuda_call(c, cudaEventElapsedTime(&ms, e0, e1));
+  for (int pass = 0; pass < 2 && !rc; ++pass) {
+    cudaEventRecord(e0, c->stream);
+    for (int r = 0; r < reps; ++r) kern<<<blocks, threads, 0, c->stream>>>(out, cap, iters, (T)1.0000001, (T)1e-9, 5);
+    cudaEventRecord(e1, c->stream);
+    c->launches += reps;
+    rc = cuda_call(c, cudaEventSynchronize(e1));
+    if (!rc) rc = cuda_call(c, cudaEventElapsedTime(&ms, e0, e1));
+    if (rc || pass == 1 || !(min_ms > (double)ms) || !(ms > 0)) break;
+    double need = min_ms / (double)ms;
+    reps = need > 4096.0 ? 4096 : (int)need + 1;
+  }
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   if (rc) return rc;
-  *fma_per_second = (double)iters * 64.0 * threads * blocks / ((double)ms * 1e-3);
-  c->launches += 2;
+  *fma_per_second = (double)reps * iters * 64.0 * threads * blocks / ((double)ms * 1e-3);
   return check(c);
 }
 
@@ -721,17 +750,20 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   // row-per-warp Euler stage; fp32 keeps the packed-f32x2 corrector and the one-thread-per-cell Euler stage
   c->corr_variant = dtype == CSPT_F64 ? 1 : 0;
   c->euler_variant = dtype == CSPT_F64 ? 1 : 0;
-  if (const char* e = getenv("CSPT_CORR")) c->corr_variant = atoi(e);        // development switches (A/B runs)
-  if (const char* e = getenv("CSPT_EULER")) c->euler_variant = atoi(e);
   c->pred_stages = 2;
-  if (const char* e = getenv("CSPT_PRED")) c->pred_stages = atoi(e);          // 0: register prefetch, 2 | 3: TMA ring depth
-  c->vac_forced = -1;
-  if (const char* e = getenv("CSPT_VAC")) c->vac_forced = atoi(e) != 0;      // force a variant (tests: both are exact)
+  c->vac_forced = -1;            // cspt_debug_force_vacuum_variant
   if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
   if (cudaEventCreateWithFlags(&c->vac_ev, cudaEventDisableTiming) != cudaSuccess) {
     (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA;
   }
   c->vac_hint = 1;
+  {
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1) {
+      (void)cudaGetLastError(); cudaEventDestroy(c->vac_ev); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA;
+    }
+    c->sm_count = sms;
+  }
   c->have_maps = dtype == CSPT_F64 ? (make_maps<double>(c) && predictor_setup<double>(c))
                                    : (make_maps<float>(c) && predictor_setup<float>(c));
   if (!c->have_maps) { (void)cudaGetLastError(); cudaEventDestroy(c->vac_ev); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA; }
@@ -876,8 +908,24 @@ int cspt_set_riemann(cspt_ctx* c, int riemann) {
                                    : euler_select<float>(c, nullptr, nullptr, nullptr);
     if (!ok) { (void)cudaGetLastError(); c->cuda_error = (int)cudaErrorUnknown; return CSPT_ECUDA; }
   }
+  // back to HLL: back to the layout a fresh ctx runs HLL on (fp32: cell per thread, with the vacuum shortcuts), so
+  // that results and speed do not depend on which solvers were selected before
+  const int fresh = c->dtype == CSPT_F64 ? 1 : 0;
+  if (riemann == CSPT_RIEMANN_HLL && c->euler_variant != fresh) {
+    c->euler_variant = fresh;
+    bool ok = c->dtype == CSPT_F64 ? euler_setup<double>(c) : euler_setup<float>(c);
+    if (!ok) { (void)cudaGetLastError(); c->cuda_error = (int)cudaErrorUnknown; return CSPT_ECUDA; }
+    drop_graphs(c);
+  }
   if (riemann != c->riemann) drop_graphs(c);
   c->riemann = riemann;
+  return CSPT_OK;
+}
+
+int cspt_debug_force_vacuum_variant(cspt_ctx* c, int force) {
+  if (!c || force < -1 || force > 1) return CSPT_EINVAL;
+  if (force != c->vac_forced) drop_graphs(c);
+  c->vac_forced = force;
   return CSPT_OK;
 }
 
@@ -922,8 +970,10 @@ int cspt_halo_put(cspt_ctx* c, int face, int what, const void* buf) {
   if (c->bc[face] != CSPT_BC_EXTERNAL) return CSPT_EINVAL;
   if (what == CSPT_HALO_U ? !c->has_state : !c->force_pending) return CSPT_ESTATE;
   if (c->cuda_error) return CSPT_ECUDA;
-  return c->dtype == CSPT_F64 ? halo_copy_t<double>(c, face, what, (void*)buf, true)
-                              : halo_copy_t<float>(c, face, what, (void*)buf, true);
+  int rc = c->dtype == CSPT_F64 ? halo_copy_t<double>(c, face, what, (void*)buf, true)
+                                : halo_copy_t<float>(c, face, what, (void*)buf, true);
+  if (!rc && what == CSPT_HALO_U) c->halo_current[face - 4] = true;
+  return rc;
 }
 
 int cspt_finish_state(cspt_ctx* c) {
@@ -943,6 +993,10 @@ int cspt_fill_ghosts(cspt_ctx* c) {
 int cspt_step_filled(cspt_ctx* c, double dt) {
   if (!c || !(dt > 0) || !isfinite(dt)) return CSPT_EINVAL;
   if (!c->has_state) return CSPT_ESTATE;
+  // the step reads the ghost layers as they are: refuse layers that belong to an earlier state
+  if (!c->ghosts_current) return CSPT_ESTATE;
+  for (int f = 4; f < 6; ++f)
+    if (c->bc[f] == CSPT_BC_EXTERNAL && !c->halo_current[f - 4]) return CSPT_ESTATE;
   if (c->cuda_error) return CSPT_ECUDA;
   return DISPATCH(c, step_filled_t)(c, dt);
 }
@@ -952,8 +1006,18 @@ int cspt_probe_fma_rate(cspt_ctx* c, int other_per_fma, double* fma_per_second) 
   if (other_per_fma != -1 && other_per_fma != 0 && other_per_fma != 1 && other_per_fma != 2 && other_per_fma != 4 && other_per_fma != 8)
     return CSPT_EINVAL;
   if (c->cuda_error) return CSPT_ECUDA;
-  return DISPATCH(c, probe_fma_t)(c, other_per_fma, fma_per_second);
+  return DISPATCH(c, probe_fma_t)(c, other_per_fma, 0.0, fma_per_second);
 }
+
+int cspt_probe_fma_rate_ms(cspt_ctx* c, int other_per_fma, double min_ms, double* fma_per_second) {
+  if (!c || !fma_per_second || !(min_ms >= 0) || !(min_ms <= 10000.0)) return CSPT_EINVAL;
+  if (other_per_fma != -1 && other_per_fma != 0 && other_per_fma != 1 && other_per_fma != 2 && other_per_fma != 4 && other_per_fma != 8)
+    return CSPT_EINVAL;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, probe_fma_t)(c, other_per_fma, min_ms, fma_per_second);
+}
+
+int cspt_sm_count(const cspt_ctx* c) { return c ? c->sm_count : 0; }
 
 int cspt_get_state(cspt_ctx* c, void* rho, void* u, void* v, void* w, void* p) {
   if (!c || !rho || !u || !v || !w || !p) return CSPT_EINVAL;

@@ -95,6 +95,7 @@ enum KernelId { K_GHOST = 0, K_PREDICTOR, K_CORRECTOR, K_EULER, K_SPEED_MAX, K_S
 struct cspt_ctx {
   cspt::Layout L;
   int dtype;
+  int sm_count;            // multiprocessors of the device that was current in cspt_create
   int bc[6];
   double h, gamma;
   void* ws;
@@ -104,6 +105,8 @@ struct cspt_ctx {
   bool has_state;
   bool force_pending;      // cspt_set_state on a slab: psi is padded, f = -D[psi] waits for cspt_finish_state
   bool smax_valid;         // smax_bits on the device belongs to the current U^n
+  bool ghosts_current;     // cspt_fill_ghosts ran on the current U^n (cspt_step_filled asks for it)
+  bool halo_current[2];    // z-lo / z-hi ghost planes were written by cspt_halo_put(CSPT_HALO_U) for the current U^n
   int cuda_error;          // sticky
   long long launches;
   void* h_pinned;          // small pinned staging buffer (scalars; byte 32: has_vac of the last cspt_set_state)
@@ -113,7 +116,7 @@ struct cspt_ctx {
   cudaEvent_t vac_ev;
   bool vac_pending;        // a copy of has_vac is in flight
   int vac_hint;            // 1: run the kernels with the shortcuts
-  int vac_forced;          // development switch CSPT_VAC: -1 = follow the hint, 0 / 1 = force the variant
+  int vac_forced;          // cspt_debug_force_vacuum_variant: -1 = follow the hint, 0 / 1 = force the variant
   int step_vac;            // the hint the step being enqueued (or captured) uses
   bool capturing;          // inside cspt_run_cfl's stream capture
   size_t elem;             // sizeof(T)

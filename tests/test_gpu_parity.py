@@ -9,7 +9,7 @@ import math
 import numpy as np
 import pytest
 
-from oracle_util import make_oracle, run_to
+from oracle_util import g9_threshold_state, make_oracle, run_to
 from paper_1912_04855_b200 import workloads as wl
 
 pytestmark = pytest.mark.gpu
@@ -284,20 +284,19 @@ def test_kernel_switch_discards_the_state_and_rejects_unknown_values(cspt, oracl
 
 
 # ---- degenerate cases ---------------------------------------------------------------------------
-def test_vacuum_shortcuts_are_exact(cspt, oracle_mod, monkeypatch):
+def test_vacuum_shortcuts_are_exact(cspt, oracle_mod):
     """The fp32 Euler stage exists with and without the gas-vacuum shortcuts (chosen by a host-side hint from
     cspt_set_state); both must give the same bits, on a workload with vacuum and on one without."""
     for w in (wl.disk(n=48), wl.random_smooth(40, 24, 20, dtype="f32")):
         got = []
-        for force in ("0", "1"):
-            monkeypatch.setenv("CSPT_VAC", force)
+        for force in (0, 1):
             s = make_solver(cspt, w)
+            s.debug_force_vacuum_variant(force)
             s.set_state(*w.fields())
             s.run_cfl(w.cfl, 6)
             s.step_cfl(w.cfl)
             got.append([t.cpu().numpy() for t in s.get_conserved()])
             s.close()
-        monkeypatch.delenv("CSPT_VAC")
         for a, b in zip(*got):
             assert np.array_equal(a, b)
         hinted = make_solver(cspt, w)                    # no override: the hint picks one of the two
@@ -490,3 +489,87 @@ def test_errors(cspt):
         assert e.value.code == cspt.EINVAL
     with pytest.raises(cspt.CsptError):
         s.compute_dt(0.0)
+
+
+# ---- round 3: ADVICE findings ---------------------------------------------------------------------
+def test_fma_probe_runs_on_the_smallest_grid(cspt):
+    """The roofline probe fills the device whatever the ctx's grid (its stores wrap around the scratch): BASELINE
+    config 1 (64x4x4) used to be refused, which lost `bench.py --workload sod` its line."""
+    import torch
+    w = wl.sod(n=64, nt=4)
+    s = make_solver(cspt, w)
+    s.set_state(*w.fields())
+    assert s.sm_count() == torch.cuda.get_device_properties(torch.cuda.current_device()).multi_processor_count
+    r = s.probe_fma_rate()
+    assert r > 1e12                                      # B200: ~1.4e13 fp64 FMA/s
+    for min_ms in (30.0, 80.0):
+        assert 0.6 < s.probe_fma_rate(0, min_ms=min_ms) / r < 1.6
+    for k in (-1, 1, 8):
+        assert s.probe_fma_rate(k) > 1e11
+    before = [t.clone() for t in s.get_conserved()]      # the probe's scratch is dead between steps
+    s.step_cfl(w.cfl)
+    big = make_solver(cspt, wl.random_smooth(96, 64, 48))
+    big.set_state(*wl.random_smooth(96, 64, 48).fields())
+    assert 0.6 < big.probe_fma_rate() / r < 1.6           # same rate from a ctx whose scratch holds the whole grid
+    fresh = make_solver(cspt, w)
+    fresh.set_state(*w.fields())
+    for a, b in zip(before, fresh.get_conserved()):
+        assert torch.equal(a, b)
+    fresh.step_cfl(w.cfl)
+    for a, b in zip(s.get_conserved(), fresh.get_conserved()):
+        assert torch.equal(a, b)
+    for x in (s, big, fresh):
+        x.close()
+
+
+def test_hll_after_another_solver_is_the_hll_of_a_fresh_ctx(cspt):
+    """cspt_set_riemann(LF | HLLC) moves an fp32 ctx to the row layout of the Euler stage; selecting HLL again moves it
+    back, so the bits of an HLL run do not depend on what was selected before (include/cspt.h)."""
+    import torch
+    for w in (wl.disk(n=40), wl.random_smooth(40, 24, 20, dtype="f32")):
+        fresh = make_solver(cspt, w)
+        fresh.set_state(*w.fields())
+        fresh.run_cfl(w.cfl, 4)
+        fresh.step_cfl(w.cfl)
+        back = make_solver(cspt, w)
+        back.set_riemann(cspt.RIEMANN_HLLC)
+        back.set_state(*w.fields())
+        back.step_cfl(w.cfl)                              # a step on the other layout, then start over with HLL
+        back.set_riemann(cspt.RIEMANN_HLL)
+        back.set_state(*w.fields())
+        back.run_cfl(w.cfl, 4)
+        back.step_cfl(w.cfl)
+        for a, b in zip(fresh.get_conserved(), back.get_conserved()):
+            assert torch.equal(a, b)
+        fresh.close()
+        back.close()
+
+
+def test_vacuum_threshold_state(cspt, oracle_mod):
+    """GPU twin of tests/test_oracle_round3_pins.py::test_vacuum_threshold_of_reading_g9: one cell just below and one
+    just above rho_vac = 1e-12 among exact vacuum.  Mask, primitives and the CFL time step bit for bit against the
+    oracle; the sub-threshold cell does not move in a step."""
+    gamma, h, cfl = 1.4, 0.1, 0.4
+    U, A, B, _ = g9_threshold_state(gamma=gamma)
+    nz, ny, nx = U[0].shape
+    zero = np.zeros_like(U[0])
+    w = wl.Workload("g9", nx, ny, nz, h, gamma, [1] * 6, (0, 0, 0), cfl, None, "f64", None)
+    o = make_oracle(oracle_mod, w)
+    o.set_state(zero, zero, zero, zero, zero, zero)
+    o.set_conserved(*U)
+    s = make_solver(cspt, w)
+    s.set_state(zero, zero, zero, zero, zero, zero)
+    s.set_conserved(*U)
+    m = s.get_vacuum_mask().cpu().numpy()
+    assert np.array_equal(m, o.get_vacuum_mask()) and m[A] == 1 and m[B] == 0
+    for a, b in zip(s.get_state(), o.get_state()):
+        assert np.array_equal(a.cpu().numpy(), b)
+    dt = s.compute_dt(cfl)
+    assert dt == o.compute_dt(cfl)
+    s.step(dt)
+    o.step(dt)
+    got = [t.cpu().numpy() for t in s.get_conserved()]
+    for q in range(5):
+        assert got[q][A] == U[q][A], q
+    assert max(field_errors(got, o.get_conserved())) < TOL64
+    s.close()

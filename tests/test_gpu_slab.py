@@ -96,10 +96,32 @@ def test_slab_protocol_errors(mods):
         with pytest.raises(cspt.CsptError) as e:
             call()                                       # a slab cannot fill its EXTERNAL faces by itself
         assert e.value.code == cspt.ESTATE
+    # cspt_step_filled refuses ghost layers that belong to an earlier state: it wants cspt_fill_ghosts and
+    # one cspt_halo_put(CSPT_HALO_U) per EXTERNAL face since the state last changed
+    def stale(call):
+        with pytest.raises(cspt.CsptError) as e:
+            call()
+        assert e.value.code == cspt.ESTATE
+    stale(lambda: s.step_filled(1e-3))                   # nothing filled yet
+    s.fill_ghosts()
+    stale(lambda: s.step_filled(1e-3))                   # no halos
+    s.halo_put(4, s.halo_get(5))
+    stale(lambda: s.step_filled(1e-3))                   # one face only
+    s.halo_put(5, s.halo_get(4))
+    s.step_filled(1e-3)                                  # complete: runs
+    stale(lambda: s.step_filled(1e-3))                   # the new state has no ghost layers
+    s.fill_ghosts()
+    s.halo_put(4, s.halo_get(5))
+    s.halo_put(5, s.halo_get(4))
+    s.set_conserved(*s.get_conserved())                  # the state changed under the halos
+    stale(lambda: s.step_filled(1e-3))
     with pytest.raises(cspt.CsptError):
         cspt.Solver(8, 8, 8, 0.1, 1.4, (cspt.BC_EXTERNAL, cspt.BC_EXTERNAL, 0, 0, 0, 0), cspt.F64)   # z faces only
     plain = cspt.Solver(8, 8, 8, 0.1, 1.4, (0,) * 6, cspt.F64)
     plain.set_state(*wl.random_smooth(8, 8, 8).fields())
+    stale(lambda: plain.step_filled(1e-3))               # also on a ctx without EXTERNAL faces
+    plain.fill_ghosts()
+    plain.step_filled(1e-3)
     with pytest.raises(cspt.CsptError) as e:
         plain.halo_put(4, plain.halo_get(5))             # face is not EXTERNAL
     assert e.value.code == cspt.EINVAL
