@@ -212,6 +212,20 @@ int cspt_halo_put(cspt_ctx*, int face, int what, const void* device_buf);
 int cspt_finish_state(cspt_ctx*);
 int cspt_fill_ghosts(cspt_ctx*);
 int cspt_step_filled(cspt_ctx*, double dt);
+/* The same protocol without the host in the time-step reduction (no sync per step):
+ *     cspt_fill_ghosts;  halo exchange;  cspt_smax_device -> max-reduce that word over the slabs IN PLACE on the
+ *     ctx's stream (e.g. ncclAllReduce, ncclMax);  cspt_step_filled_cfl(cfl)
+ * cspt_smax_device: evaluates the maximum signal speed max_cells(c + max(|u|,|v|,|w|)) of this slab (reading G15) if
+ *   it is not already known from the last step's Euler stage, and returns the DEVICE address of the word that holds it:
+ *   one element of the ctx's dtype (double / float), non-negative, 0 for an all-vacuum slab, valid once the ctx's
+ *   stream reaches this point.  The maximum over the slabs, written back to the same word, is what the undivided grid
+ *   would hold: non-negative IEEE numbers order like their bit patterns, so a floating-point max-reduction is exact.
+ *   The word lives in the ctx's workspace; it is consumed (reset) by the next step.
+ * cspt_step_filled_cfl: dt = (cfl*h)/that word (+inf -> identity step), then S1..S9 as cspt_step_filled.
+ *   dt_host_out may be NULL; if not, dt is written there and the call syncs.  ESTATE: as cspt_step_filled, or
+ *   cspt_smax_device was not called for the current state.  EINVAL: cfl <= 0 or not finite. */
+int cspt_smax_device(cspt_ctx*, void** device_ptr);
+int cspt_step_filled_cfl(cspt_ctx*, double cfl, double* dt_host_out);
 /* ---- CFL time step without a ctx, a workspace or any allocation ------------------------------------------------
  * For callers that cannot allocate device memory.  cspt_compute_dt needs a ctx, and a ctx needs a workspace of 28
  * padded fields that someone must allocate.  That is impossible for a host code that gave all of HBM to its own arena

@@ -54,6 +54,8 @@ SYMBOLS = [
     ("cspt_finish_state", _ci, [_vp]),
     ("cspt_fill_ghosts", _ci, [_vp]),
     ("cspt_step_filled", _ci, [_vp, _cd]),
+    ("cspt_smax_device", _ci, [_vp, ctypes.POINTER(_vp)]),
+    ("cspt_step_filled_cfl", _ci, [_vp, _cd, _pd]),
     ("cspt_noalloc_max_cells", ctypes.c_longlong, []),
     ("cspt_cfl_dt_noalloc", _ci, [_ci, ctypes.c_longlong, _vp, _vp, _vp, _vp, _vp, _cd, _cd, _cd, _vp, _vp]),
     ("cspt_cuda_error", _ci, [_vp]),
@@ -336,6 +338,27 @@ class Solver:
 
     def step_filled(self, dt):
         _check(lib().cspt_step_filled(self._h, float(dt)), "cspt_step_filled")
+
+    def smax_device(self):
+        """The slab's maximum signal speed as a one-element tensor VIEW of the word in the workspace (no copy): reduce
+        it in place over the slabs (all_reduce MAX on the solver's stream), then step_filled_cfl."""
+        p = ctypes.c_void_p()
+        self._before()
+        _check(lib().cspt_smax_device(self._h, ctypes.byref(p)), "cspt_smax_device")
+        self._after()
+        off = p.value - self.workspace.data_ptr()
+        esz = 8 if self.dtype == F64 else 4
+        assert 0 <= off and off + esz <= self.workspace.numel() and off % esz == 0
+        return self.workspace[off:off + esz].view(self.tdtype)
+
+    def step_filled_cfl(self, cfl, want_dt=False):
+        self._before()
+        if want_dt:
+            out = ctypes.c_double()
+            _check(lib().cspt_step_filled_cfl(self._h, float(cfl), ctypes.byref(out)), "cspt_step_filled_cfl")
+            return out.value
+        _check(lib().cspt_step_filled_cfl(self._h, float(cfl), None), "cspt_step_filled_cfl")
+        return None
 
     def cuda_error(self):
         return int(lib().cspt_cuda_error(self._h))

@@ -551,6 +551,29 @@ int step_filled_t(cspt_ctx* c, double dt) {
   return check(c);
 }
 
+// slab path: the signal-speed maximum stays on the device, the caller max-reduces it over the slabs in place
+template <class T>
+int smax_device_t(cspt_ctx* c, void** ptr) {
+  ensure_smax<T>(c);
+  *ptr = &scalars<T>(c)->smax_bits;
+  return check(c);
+}
+
+template <class T>
+int step_filled_cfl_t(cspt_ctx* c, double cfl, double* out) {
+  LAUNCH(c, K_SCALAR, k_dt_finalize<T>, 1, 1, scalars<T>(c), (T)cfl, (T)c->h);
+  run_step<T>(c, false);
+  int rc = check(c);
+  if (rc || !out) return rc;
+  T* hb = (T*)c->h_pinned;
+  rc = cuda_call(c, cudaMemcpyAsync(hb, &scalars<T>(c)->dt, sizeof(T), cudaMemcpyDeviceToHost, c->stream));
+  if (rc) return rc;
+  rc = cuda_call(c, cudaStreamSynchronize(c->stream));
+  if (rc) return rc;
+  *out = (double)*hb;
+  return CSPT_OK;
+}
+
 template <class T>
 int step_cfl_t(cspt_ctx* c, double cfl, double* out) {
   ensure_smax<T>(c);
@@ -999,6 +1022,23 @@ int cspt_step_filled(cspt_ctx* c, double dt) {
     if (c->bc[f] == CSPT_BC_EXTERNAL && !c->halo_current[f - 4]) return CSPT_ESTATE;
   if (c->cuda_error) return CSPT_ECUDA;
   return DISPATCH(c, step_filled_t)(c, dt);
+}
+
+int cspt_smax_device(cspt_ctx* c, void** device_ptr) {
+  if (!c || !device_ptr) return CSPT_EINVAL;
+  if (!c->has_state) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, smax_device_t)(c, device_ptr);
+}
+
+int cspt_step_filled_cfl(cspt_ctx* c, double cfl, double* dt_host_out) {
+  if (!c || !(cfl > 0) || !isfinite(cfl)) return CSPT_EINVAL;
+  if (!c->has_state || !c->smax_valid) return CSPT_ESTATE;      // cspt_smax_device first
+  if (!c->ghosts_current) return CSPT_ESTATE;
+  for (int f = 4; f < 6; ++f)
+    if (c->bc[f] == CSPT_BC_EXTERNAL && !c->halo_current[f - 4]) return CSPT_ESTATE;
+  if (c->cuda_error) return CSPT_ECUDA;
+  return DISPATCH(c, step_filled_cfl_t)(c, cfl, dt_host_out);
 }
 
 int cspt_probe_fma_rate(cspt_ctx* c, int other_per_fma, double* fma_per_second) {

@@ -83,6 +83,20 @@ class DistTransport:
             for req in dist.batch_isend_irecv(ops):
                 req.wait()
 
+    @property
+    def stream_ordered(self):
+        """True when the backend enqueues its transfers on CUDA streams ordered after torch's current stream (NCCL)."""
+        try:
+            return self.world > 1 and self.dist.get_backend(self.group) == "nccl"
+        except Exception:
+            return False
+
+    def max_scalar(self, t):
+        """In-place maximum over all ranks of a one-element tensor."""
+        if self.world > 1:
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX, group=self.group)
+        return t
+
     def min_scalar(self, t):
         """In-place minimum over all ranks of a one-element tensor."""
         if self.world > 1:
@@ -104,10 +118,10 @@ class _Slab:
         """This slab's planes of arrays given on the whole grid (nz, ny, nx)."""
         return [f[self.z0:self.z1] for f in fields]
 
-    def _get(self, what):
+    def _get(self, what, out=(None, None)):
         s = self.solver
-        return (s.halo_get(FACE_ZLO, what) if self.lo is not None else None,
-                s.halo_get(FACE_ZHI, what) if self.hi is not None else None)
+        return (s.halo_get(FACE_ZLO, what, out[0]) if self.lo is not None else None,
+                s.halo_get(FACE_ZHI, what, out[1]) if self.hi is not None else None)
 
     def _put(self, what, recv_lo, recv_hi):
         if self.lo is not None:
@@ -127,13 +141,21 @@ class SlabSolver(_Slab):
     def __init__(self, nx, ny, nz_global, h, gamma, bc, dtype=cspt.F64, rank=0, world=1, transport=None, stream=None):
         super().__init__(nx, ny, nz_global, h, gamma, bc, dtype, rank, world, stream)
         self.transport = transport or DistTransport(bc, rank, world)
+        self._bufs = {}
 
     def _exchange(self, what):
-        send_lo, send_hi = self._get(what)
-        recv_lo, recv_hi = self._buffers(what)
-        self.solver.torch.cuda.current_stream().synchronize()     # the messages are complete before they leave
-        self.transport.exchange(send_lo, send_hi, recv_lo, recv_hi)
-        self._put(what, recv_lo, recv_hi)
+        # message buffers are allocated once per kind of message and reused every step
+        if what not in self._bufs:
+            self._bufs[what] = (self._buffers(what), self._buffers(what))
+        send, recv = self._bufs[what]
+        send_lo, send_hi = self._get(what, send)
+        # NCCL orders its send/recv after the work already enqueued on torch's current stream (which halo_get made
+        # wait for the solver's stream) and makes that stream wait for their completion: no host synchronisation.
+        # Any other backend gets the messages only once they are complete.
+        if not getattr(self.transport, "stream_ordered", False):
+            self.solver.torch.cuda.current_stream().synchronize()
+        self.transport.exchange(send_lo, send_hi, recv[0], recv[1])
+        self._put(what, recv[0], recv[1])
 
     def set_state(self, rho, u, v, w, p, psi):
         """Arrays of THIS slab, (z1 - z0, ny, nx)."""
@@ -142,14 +164,18 @@ class SlabSolver(_Slab):
             self._exchange(cspt.HALO_PSI)
             self.solver.finish_state()
 
-    def step_cfl(self, cfl):
+    def step_cfl(self, cfl, want_dt=True):
+        """One CFL-limited step of the whole grid.  The time step never visits the host: the slab's maximum signal
+        speed is max-reduced over the ranks in place on the device (a view of the word in the solver's workspace) and
+        cspt_step_filled_cfl forms dt from it.  want_dt=False enqueues only (no host synchronisation in the step);
+        want_dt=True (default) also returns dt, which waits for the step."""
         s = self.solver
         s.fill_ghosts()
         self._exchange(cspt.HALO_U)
-        t = s.torch.tensor([s.compute_dt(cfl)], dtype=s.torch.float64, device=s.device)
-        dt = float(self.transport.min_scalar(t).item())
-        s.step_filled(dt)
-        return dt
+        smax = s.smax_device()
+        self.transport.max_scalar(smax)
+        s.stream.wait_stream(s.torch.cuda.current_stream())     # the reduced word is in place before dt is formed
+        return s.step_filled_cfl(cfl, want_dt)
 
     def get_conserved(self):
         return self.solver.get_conserved()
@@ -182,14 +208,30 @@ class LocalSlabs:
             for sl in self.slabs:
                 sl.solver.finish_state()
 
-    def step_cfl(self, cfl):
+    def step_cfl(self, cfl, device_dt=False):
+        """device_dt=False: dt = min over slabs of cspt_compute_dt on the host, then cspt_step_filled(dt).
+        device_dt=True: the phases of SlabSolver.step_cfl: the slabs' signal-speed words are max-reduced on the device
+        (here a torch.maximum over the views, standing in for the all-reduce) and cspt_step_filled_cfl forms dt."""
         for sl in self.slabs:
             sl.solver.fill_ghosts()
         self._exchange(cspt.HALO_U)
-        dt = min(sl.solver.compute_dt(cfl) for sl in self.slabs)
+        if not device_dt:
+            dt = min(sl.solver.compute_dt(cfl) for sl in self.slabs)
+            for sl in self.slabs:
+                sl.solver.step_filled(dt)
+            return dt
+        words = [sl.solver.smax_device() for sl in self.slabs]
+        top = words[0].clone()
+        for wd in words[1:]:
+            top = self.slabs[0].solver.torch.maximum(top, wd)
+        for wd in words:
+            wd.copy_(top)
+        dts = []
         for sl in self.slabs:
-            sl.solver.step_filled(dt)
-        return dt
+            sl.solver.stream.wait_stream(sl.solver.torch.cuda.current_stream())
+            dts.append(sl.solver.step_filled_cfl(cfl, want_dt=True))
+        assert all(d == dts[0] for d in dts)
+        return dts[0]
 
     def get_conserved(self):
         torch = self.slabs[0].solver.torch

@@ -23,7 +23,7 @@ def mods():
     return cspt, slab
 
 
-def _run_both(cspt, slab, w, world, steps, dtype=None):
+def _run_both(cspt, slab, w, world, steps, dtype=None, device_dt=False):
     d = cspt.F64 if (dtype or w.dtype) == "f64" else cspt.F32
     f = w.fields() if dtype is None else [a.astype(np.float32 if dtype == "f32" else np.float64) for a in w.fields()]
     one = cspt.Solver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, d)
@@ -33,7 +33,7 @@ def _run_both(cspt, slab, w, world, steps, dtype=None):
     dts = []
     for _ in range(steps):
         dt1 = one.step_cfl(w.cfl, want_dt=True)
-        dt2 = many.step_cfl(w.cfl)
+        dt2 = many.step_cfl(w.cfl, device_dt=device_dt)
         assert dt1 == dt2                     # min over the slabs of the local CFL steps is the grid's step, bit for bit
         dts.append(dt1)
     a = [t.cpu().numpy() for t in one.get_conserved()]
@@ -51,6 +51,61 @@ def test_slabs_advance_exactly_as_the_undivided_grid(mods, bc, world):
     _, a, b, _ = _run_both(cspt, slab, w, world, 10)
     for q in range(5):
         assert np.array_equal(a[q], b[q]), (q, float(np.max(np.abs(a[q] - b[q]))))
+
+
+@pytest.mark.parametrize("world,bc,dtype", [(2, (P, P, P, P, P, P), None), (3, (I, O, P, P, O, O), None),
+                                            (3, (O, O, O, O, I, O), "f32")])
+def test_time_step_reduced_on_the_device(mods, world, bc, dtype):
+    """The sync-free protocol of SlabSolver.step_cfl (cspt_smax_device -> max over the slabs in place ->
+    cspt_step_filled_cfl) gives the time step and the state of the undivided grid, bit for bit."""
+    cspt, slab = mods
+    w = wl.random_smooth(40, 12, 26, bc=bc)
+    _, a, b, _ = _run_both(cspt, slab, w, world, 8, dtype=dtype, device_dt=True)
+    for q in range(5):
+        assert np.array_equal(a[q], b[q]), q
+
+
+def _nccl_rank(rank, world, port, nz, out_path):
+    import os
+    import torch
+    import torch.distributed as dist
+    from paper_1912_04855_b200 import cspt, slab
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    torch.cuda.set_device(rank)
+    dist.init_process_group("nccl", rank=rank, world_size=world, device_id=torch.device("cuda", rank))
+    w = wl.random_smooth(40, 12, nz, bc=(P, P, P, P, P, P))
+    s = slab.SlabSolver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, cspt.F64, rank, world)
+    s.set_state(*s.local(w.fields()))
+    dts = [s.step_cfl(w.cfl) for _ in range(6)]
+    s.step_cfl(w.cfl, want_dt=False)                  # the sync-free form
+    dts.append(None)
+    mine = torch.stack(s.get_conserved()).cpu()
+    torch.save({"z0": s.z0, "z1": s.z1, "U": mine, "dts": dts}, "%s.%d" % (out_path, rank))
+    s.close()
+    dist.destroy_process_group()
+
+
+def test_slab_solver_over_nccl_on_two_gpus(mods, tmp_path):
+    """The real transport: one process per GPU, NCCL send/recv of the halos and an NCCL max-reduction of the signal
+    speed.  Needs two GPUs (skipped otherwise); bit-equality with the undivided grid."""
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs 2 GPUs")
+    import torch.multiprocessing as mp
+    cspt, slab = mods
+    nz, world = 26, 2
+    out = str(tmp_path / "slab")
+    mp.spawn(_nccl_rank, args=(world, 29533, nz, out), nprocs=world, join=True)
+    w = wl.random_smooth(40, 12, nz, bc=(P, P, P, P, P, P))
+    one = cspt.Solver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, cspt.F64)
+    one.set_state(*w.fields())
+    dts = [one.step_cfl(w.cfl, want_dt=True) for _ in range(7)]
+    ref = torch.stack(one.get_conserved()).cpu()
+    for r in range(world):
+        d = torch.load("%s.%d" % (out, r))
+        assert d["dts"][:6] == dts[:6]
+        assert torch.equal(d["U"], ref[:, d["z0"]:d["z1"]])
+    one.close()
 
 
 def test_slabs_fp32_and_disk_vacuum(mods):
