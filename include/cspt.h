@@ -182,6 +182,14 @@ int cspt_sm_count(const cspt_ctx*);
  * give the same bits.  force = 0 / 1 pins the variant without / with the shortcuts (the test of that equality),
  * -1 follows the hint again.  Host-side only.  EINVAL: null ctx, force not in {-1, 0, 1}. */
 int cspt_debug_force_vacuum_variant(cspt_ctx*, int force);
+/* CTA-level gas-vacuum shortcut of the fp32 kernels: a CTA whose inputs within the 3-cell reach
+ * of a step are all exactly 0, according to a device-resident map of bricks that have held gas, writes its exactly-zero
+ * results and returns before its first load.  on = 0 switches it off (the test of bit equality with the full
+ * evaluation), 1 (default) on.  Host-side only.  EINVAL: null ctx, on not 0 or 1. */
+int cspt_debug_tile_skip(cspt_ctx*, int on);
+/* CTAs that took that early return since the map was last rebuilt (cspt_set_state, cspt_set_conserved, a switch of
+ * variant), 0 if no map is in use.  Syncs. */
+int cspt_debug_dead_ctas(cspt_ctx*, long long* count);
 /* ---- end of diagnostics ------------------------------------------------------------------------------------------ */
 /* ---- z-slab decomposition over several GPUs ("the computational domain is divided between GPUs",
  * :123).  One ctx per slab of nz_local planes; a z face that borders another slab has

@@ -48,6 +48,8 @@ SYMBOLS = [
     ("cspt_probe_fma_rate_ms", _ci, [_vp, _ci, _cd, _pd]),
     ("cspt_sm_count", _ci, [_vp]),
     ("cspt_debug_force_vacuum_variant", _ci, [_vp, _ci]),
+    ("cspt_debug_tile_skip", _ci, [_vp, _ci]),
+    ("cspt_debug_dead_ctas", _ci, [_vp, ctypes.POINTER(ctypes.c_longlong)]),
     ("cspt_halo_elems", _ci, [_vp, _ci, ctypes.POINTER(ctypes.c_longlong)]),
     ("cspt_halo_get", _ci, [_vp, _ci, _ci, _vp]),
     ("cspt_halo_put", _ci, [_vp, _ci, _ci, _vp]),
@@ -303,6 +305,14 @@ class Solver:
         else:
             _check(lib().cspt_probe_fma_rate(self._h, int(other_per_fma), ctypes.byref(out)), "cspt_probe_fma_rate")
         return out.value
+
+    def debug_tile_skip(self, on):
+        _check(lib().cspt_debug_tile_skip(self._h, 1 if on else 0), "cspt_debug_tile_skip")
+
+    def debug_dead_ctas(self):
+        n = ctypes.c_longlong()
+        _check(lib().cspt_debug_dead_ctas(self._h, ctypes.byref(n)), "cspt_debug_dead_ctas")
+        return int(n.value)
 
     def debug_force_vacuum_variant(self, force):
         _check(lib().cspt_debug_force_vacuum_variant(self._h, int(force)), "cspt_debug_force_vacuum_variant")

@@ -37,6 +37,18 @@ void carve(cspt_ctx* c) {
   c->inflow_plane = inflow_plane_elems(c->L);
   c->off_inflow = align_up((size_t)S_COUNT * c->L.fstride * e, 256);
   c->off_scalars = align_up(c->off_inflow + (size_t)6 * 5 * c->inflow_plane * e, 256);
+  c->off_map = c->off_scalars + 256;
+  c->map_bytes = 256 + align_up((size_t)((c->L.px + BRX - 1) / BRX) * ((c->L.py + BRY - 1) / BRY) * ((c->L.pz + BRZ - 1) / BRZ), 256);
+}
+
+// the brick map of the CTA-level gas-vacuum shortcut (cspt_common.cuh); on = false: a map that switches it off
+inline BrickMap brick_map(const cspt_ctx* c, bool on) {
+  BrickMap M;
+  M.raw = on ? (unsigned char*)c->ws + c->off_map + 256 : nullptr;      // first 256 bytes: the diagnostics counter
+  M.dead = (unsigned long long*)((unsigned char*)c->ws + c->off_map);
+  M.zero_fill = c->zero_fill_steps > 0 ? 1 : 0;
+  M.nbx = (c->L.px + BRX - 1) / BRX; M.nby = (c->L.py + BRY - 1) / BRY; M.nbz = (c->L.pz + BRZ - 1) / BRZ;
+  return M;
 }
 
 template <class T> T* field(cspt_ctx* c, int slot) { return (T*)((char*)c->ws + c->off_fields) + (long long)slot * c->L.fstride; }
@@ -109,7 +121,7 @@ int cuda_call(cspt_ctx* c, cudaError_t e) {
 
 // ---- ghost layers, x then y then z (G16) ----------------------------------------------
 template <class T>
-void fill_ghosts(cspt_ctx* c, T* F, int nfields, int mode) {
+void fill_ghosts(cspt_ctx* c, T* F, int nfields, int mode, BrickMap M = BrickMap{nullptr, 0, 0, 0, nullptr, 1}) {
   const Layout& L = c->L;
   int n[3] = {L.nx, L.ny, L.nz};
   for (int d = 0; d < 3; ++d) {
@@ -117,7 +129,7 @@ void fill_ghosts(cspt_ctx* c, T* F, int nfields, int mode) {
     long long e1 = d1 < d ? n[d1] + 2 * NG : n[d1], e2 = d2 < d ? n[d2] + 2 * NG : n[d2];
     long long total = e1 * e2 * NG * 2;
     LAUNCH(c, K_GHOST, k_ghost_axis<T>, blocks_for(total, TPB, STRIDE_CAP), TPB, L, d, mode, c->bc[2 * d], c->bc[2 * d + 1],
-           nfields, F, inflow<T>(c, 2 * d), inflow<T>(c, 2 * d + 1), c->inflow_plane);
+           nfields, F, inflow<T>(c, 2 * d), inflow<T>(c, 2 * d + 1), c->inflow_plane, M);
   }
 }
 
@@ -164,7 +176,8 @@ int halo_copy_t(cspt_ctx* c, int face, int what, void* buf, bool put) {
 
 template <class T>
 int fill_ghosts_t(cspt_ctx* c) {
-  fill_ghosts<T>(c, field<T>(c, c->cur ? S_U1 : S_U0), 5, 0);
+  // a valid brick map keeps following the gas (flags are only added; an invalid one is rebuilt from the filled array)
+  fill_ghosts<T>(c, field<T>(c, c->cur ? S_U1 : S_U0), 5, 0, brick_map(c, c->dtype == CSPT_F32 && c->map_valid));
   c->ghosts_current = true;
   return check(c);
 }
@@ -190,6 +203,7 @@ int set_state_t(cspt_ctx* c, const void* rho, const void* u, const void* v, cons
   c->smax_valid = false;
   c->has_state = false;
   c->force_pending = true;
+  c->map_valid = false;
   stale_ghosts(c);
   // a slab (EXTERNAL z faces) needs the psi ghost planes of its neighbours before f = -D[psi] can be formed there:
   // cspt_halo_get/put(CSPT_HALO_PSI), then cspt_finish_state
@@ -206,6 +220,7 @@ int set_conserved_t(cspt_ctx* c, const void* const in[5]) {
   c->vac_pending = false;        // the new state was not looked at: keep the shortcuts on
   c->vac_hint = 1;
   c->smax_valid = false;
+  c->map_valid = false;
   stale_ghosts(c);
   return check(c);
 }
@@ -263,6 +278,27 @@ int compute_dt_t(cspt_ctx* c, double cfl, double* out) {
 constexpr int ETX = 32;
 template <class T> struct EulerTile { static constexpr int TY = 8; };
 
+// CTA-level gas-vacuum shortcut (BrickMap): only the fp32 streaming kernels carry it, the map follows the gas through
+// the flags of the ghost fill and of the cell-per-thread Euler stage, and it pays only where the state holds vacuum
+inline bool tile_skip_on(const cspt_ctx* c) {
+  return c->dtype == CSPT_F32 && c->euler_variant == 0 && c->step_vac != 0 && c->tile_skip != 0 &&
+         c->bc[4] != CSPT_BC_EXTERNAL && c->bc[5] != CSPT_BC_EXTERNAL;
+}
+inline BrickMap step_map(const cspt_ctx* c) { return brick_map(c, tile_skip_on(c)); }
+
+// the map must cover every non-zero cell of the current U^n before a step may rely on it: rebuilt (one read of U) after
+// cspt_set_state / cspt_set_conserved and after steps that ran without the flags
+template <class T>
+void ensure_map(cspt_ctx* c) {
+  if (c->map_valid || !tile_skip_on(c)) return;
+  BrickMap M = brick_map(c, true);
+  cudaMemsetAsync(M.dead, 0, c->map_bytes, c->stream);      // counter and flags
+  long long n = (long long)(c->L.nx + 2 * NG) * (c->L.ny + 2 * NG) * (c->L.nz + 2 * NG);
+  LAUNCH(c, K_IO, k_brick_scan<T>, blocks_for(n, TPB, STRIDE_CAP), TPB, c->L, field<T>(c, c->cur ? S_U1 : S_U0), M);
+  c->map_valid = true;
+  c->zero_fill_steps = 2;
+}
+
 int pick_zchunk(int tiles, int nz) {
   // enough CTAs for ~8 waves of 2 CTAs per SM, at least 16 planes per CTA (2 extra planes per chunk) and at
   // most 64: CTAs of neighbouring tiles then stay close in z, so the halo rows they share are still in L2
@@ -301,7 +337,7 @@ bool corr_variant(cspt_ctx* c, const Params<T>* P, const T* U) {
   dim3 grid(gx, gy, (L.nz + 2 + zc - 1) / zc);
   int ps_ = prof_open(c, K_CORRECTOR);
   kern<<<grid, SC::THREADS, SC::BYTES, c->stream>>>(c->mapS, *P, scalars<T>(c), U, field<T>(c, S_F), field<T>(c, S_ST),
-                                                     field<T>(c, S_UT), field<T>(c, S_XI), zc);
+                                                     field<T>(c, S_UT), field<T>(c, S_XI), zc, step_map(c));
   prof_close(c, ps_);
   c->launches++;
   return true;
@@ -449,7 +485,7 @@ void launch_predictor(cspt_ctx* c, const Params<T>& P, const T* U) {
   int ps_ = prof_open(c, K_PREDICTOR);
   auto launch = [&](auto kern, int bytes) {
     kern<<<grid, PTX * PTY, bytes, c->stream>>>(c->mapPU[c->cur], c->mapPF, P, scalars<T>(c), U, field<T>(c, S_F),
-                                                 field<T>(c, S_ST), zc, x0, x1);
+                                                 field<T>(c, S_ST), zc, x0, x1, step_map(c));
   };
   launch(k_predictor_stream<T, PTX, PTY, 2>, PredRing<T, PTX, PTY, 2>::BYTES);
   prof_close(c, ps_);
@@ -507,7 +543,7 @@ void launch_euler(cspt_ctx* c, const Params<T>& P, const T* U, T* UN) {
   const bool vl = c->limiter == CSPT_LIMITER_VANLEER, vac = c->step_vac != 0;
   auto kern = vac ? (vl ? k_euler_stream<T, ETX, ETY, 1, 1> : k_euler_stream<T, ETX, ETY, 0, 1>)
                   : (vl ? k_euler_stream<T, ETX, ETY, 1, 0> : k_euler_stream<T, ETX, ETY, 0, 0>);
-  kern<<<grid, ETX * ETY, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN, &sc->smax_bits, zc);
+  kern<<<grid, ETX * ETY, S::BYTES, c->stream>>>(c->mapU[c->cur], c->mapL, P, sc, U, UN, &sc->smax_bits, zc, step_map(c));
   prof_close(c, ps_);
   c->launches++;
   }
@@ -524,17 +560,19 @@ void wait_pending_output(cspt_ctx* c) {
 template <class T>
 void run_step(cspt_ctx* c, bool fill = true) {
   wait_pending_output(c);
-  if (!c->capturing) c->step_vac = vacuum_hint(c);
+  if (!c->capturing) { c->step_vac = vacuum_hint(c); ensure_map<T>(c); }
   Params<T> P = make_params<T>(c);
   T* U = field<T>(c, c->cur ? S_U1 : S_U0);
   T* UN = field<T>(c, c->cur ? S_U0 : S_U1);
-  if (fill) fill_ghosts<T>(c, U, 5, 0);                                            // O0
+  if (fill) fill_ghosts<T>(c, U, 5, 0, step_map(c));                               // O0
   launch_predictor<T>(c, P, U);                                                    // O1, O3, O4
   launch_corrector<T>(c, P, U);                                                    // O5, O6
   launch_euler<T>(c, P, U, UN);                                                  // O7, O8 (+O9 epilogue)
   c->cur ^= 1;
   c->smax_valid = true;
   stale_ghosts(c);               // U^{n+1} has no ghost layers yet
+  if (!tile_skip_on(c)) c->map_valid = false;      // this step did not flag where its gas went
+  else if (c->zero_fill_steps > 0) c->zero_fill_steps--;
 }
 
 template <class T>
@@ -613,6 +651,7 @@ int capture_two_steps(cspt_ctx* c, double cfl) {
   cudaStream_t gs = graph_stream(c), user = c->stream;
   if (!gs) { c->cuda_error = (int)cudaErrorUnknown; return CSPT_ECUDA; }
   c->step_vac = c->graph_vac = vacuum_hint(c);
+  ensure_map<T>(c);                                  // on the ctx's stream, ahead of the capture (the graph only adds flags)
   int rc = cuda_call(c, cudaStreamBeginCapture(gs, cudaStreamCaptureModeThreadLocal));
   if (rc) return rc;
   c->capturing = true;
@@ -641,12 +680,25 @@ int run_cfl_t(cspt_ctx* c, double cfl, int nsteps, double* t_out) {
   int rc = check(c);
   if (rc) return rc;
   int left = nsteps;
+  // CTA-level vacuum shortcut: the graphs bake in "the zeros of dead CTAs are in place", which holds once two plain
+  // steps have written them (after the map was rebuilt or the intermediate slots served as staging)
+  if (!c->prof_on && left >= 2) {
+    c->step_vac = vacuum_hint(c);
+    if (tile_skip_on(c)) {
+      ensure_map<T>(c);
+      for (; left > 0 && c->zero_fill_steps > 0; --left) {
+        LAUNCH(c, K_SCALAR, k_dt_finalize<T>, 1, 1, scalars<T>(c), (T)cfl, (T)c->h);
+        run_step<T>(c);
+      }
+    }
+  }
   if (!c->prof_on && left >= 2) {                    // event pairs cannot be recorded inside a graph: plain loop then
     if ((c->graph[0] || c->graph[1]) && (c->graph_cfl != cfl || c->graph_vac != vacuum_hint(c))) drop_graphs(c);
     if (!c->graph[c->cur]) {
       rc = capture_two_steps<T>(c, cfl);
       if (rc) return rc;
     }
+    c->step_vac = c->graph_vac;
     const long long per_pair = 2 * 7;                // 3 ghost fills, predictor, corrector, Euler stage, dt
     for (; left >= 2; left -= 2) {
       rc = cuda_call(c, cudaGraphLaunch(c->graph[c->cur], graph_stream(c)));
@@ -674,6 +726,7 @@ int probe_fma_t(cspt_ctx* c, int other_per_fma, double min_ms, double* fma_per_s
   // scratch: the star-group slots are dead between steps; the kernel's stores are a sink that wraps around it, so
   // the grid always fills the device (8 CTAs of 128 threads per SM), whatever the size of the ctx's grid
   T* out = field<T>(c, S_ST);
+  c->zero_fill_steps = 2;          // the sink overwrites slots that dead CTAs rely on
   const int threads = 128, blocks = c->sm_count * 8, iters = other_per_fma ? 1500 : 4000;
   long long room = c->L.fstride * 8, want = (long long)threads * blocks;
   const unsigned cap = (unsigned)(room < want ? room : want);
@@ -738,7 +791,7 @@ size_t cspt_workspace_bytes(int nx, int ny, int nz, int dtype) {
   tmp.L = make_layout(nx, ny, nz);
   tmp.elem = elem_size(dtype);
   carve(&tmp);
-  return tmp.off_scalars + 256;
+  return tmp.off_map + tmp.map_bytes;
 }
 
 int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, const int bc[6], int dtype,
@@ -775,6 +828,7 @@ int cspt_create(cspt_ctx** out, int nx, int ny, int nz, double h, double gamma, 
   c->euler_variant = dtype == CSPT_F64 ? 1 : 0;
   c->pred_stages = 2;
   c->vac_forced = -1;            // cspt_debug_force_vacuum_variant
+  c->tile_skip = 1;              // cspt_debug_tile_skip
   if (cudaMallocHost(&c->h_pinned, 64) != cudaSuccess) { (void)cudaGetLastError(); delete c; return CSPT_ECUDA; }
   if (cudaEventCreateWithFlags(&c->vac_ev, cudaEventDisableTiming) != cudaSuccess) {
     (void)cudaGetLastError(); cudaFreeHost(c->h_pinned); delete c; return CSPT_ECUDA;
@@ -945,6 +999,25 @@ int cspt_set_riemann(cspt_ctx* c, int riemann) {
   return CSPT_OK;
 }
 
+int cspt_debug_dead_ctas(cspt_ctx* c, long long* count) {
+  if (!c || !count) return CSPT_EINVAL;
+  if (c->cuda_error) return CSPT_ECUDA;
+  *count = 0;
+  if (!c->map_valid) return CSPT_OK;
+  unsigned long long* hb = (unsigned long long*)c->h_pinned;
+  int rc = cuda_call(c, cudaMemcpyAsync(hb, (unsigned char*)c->ws + c->off_map, 8, cudaMemcpyDeviceToHost, c->stream));
+  if (!rc) rc = cuda_call(c, cudaStreamSynchronize(c->stream));
+  if (!rc) *count = (long long)*hb;
+  return rc;
+}
+
+int cspt_debug_tile_skip(cspt_ctx* c, int on) {
+  if (!c || (on != 0 && on != 1)) return CSPT_EINVAL;
+  if (on != c->tile_skip) { drop_graphs(c); c->map_valid = false; }
+  c->tile_skip = on;
+  return CSPT_OK;
+}
+
 int cspt_debug_force_vacuum_variant(cspt_ctx* c, int force) {
   if (!c || force < -1 || force > 1) return CSPT_EINVAL;
   if (force != c->vac_forced) drop_graphs(c);
@@ -1080,6 +1153,7 @@ int cspt_get_conserved_host(cspt_ctx* c, void* rho, void* mx, void* my, void* mz
   if (c->cuda_error) return CSPT_ECUDA;
   void* host[5] = {rho, mx, my, mz, E};
   void* dev[5];
+  c->zero_fill_steps = 2;          // the staging arrays overwrite intermediate slots that dead CTAs rely on
   for (int f = 0; f < 5; ++f) dev[f] = c->dtype == CSPT_F64 ? (void*)staging<double>(c, f) : (void*)staging<float>(c, f);
   int rc = DISPATCH(c, get_conserved_t)(c, dev);
   if (rc) return rc;
@@ -1099,6 +1173,7 @@ int cspt_get_conserved_host_async(cspt_ctx* c, void* rho, void* mx, void* my, vo
   wait_pending_output(c);                     // an earlier result still leaving through the same staging slots
   void* host[5] = {rho, mx, my, mz, E};
   void* dev[5];
+  c->zero_fill_steps = 2;          // the staging arrays overwrite intermediate slots that dead CTAs rely on
   for (int f = 0; f < 5; ++f) dev[f] = c->dtype == CSPT_F64 ? (void*)staging_out<double>(c, f) : (void*)staging_out<float>(c, f);
   int rc = DISPATCH(c, get_conserved_t)(c, dev);
   if (rc) return rc;

@@ -43,6 +43,20 @@ inline Layout make_layout(int nx, int ny, int nz) {
   return L;
 }
 
+// Gas-vacuum handling at CTA level (fp32 streaming kernels): a byte per BRX x BRY x BRZ brick of the PADDED array,
+// non-zero once any of rho, m, E was non-zero in a cell of the brick since the map was last rebuilt (flags are only
+// ever added: a brick that held gas stays "live").  One full step reaches 3 cells, so a CTA whose output footprint,
+// widened by 3 cells, touches no live brick has inputs that are exactly 0 and outputs that are exactly 0: it writes
+// those zeros and returns before its first load.  raw == nullptr: off.
+constexpr int BRX = 32, BRY = 8, BRZ = 8;
+struct BrickMap {
+  unsigned char* raw;
+  int nbx, nby, nbz;
+  unsigned long long* dead;      // diagnostics: CTAs that returned early since the map was last rebuilt
+  int zero_fill;                 // 1: a dead CTA writes its zeros; 0: they are known to be in place already (it was
+                                 // dead in the last two steps too and nothing else has touched the buffers since)
+};
+
 // Field slots inside the workspace (each fstride elements of T).
 enum Slot {
   S_U0 = 0,        // U buffer A: rho, mx, my, mz, E          (5)
@@ -121,7 +135,12 @@ struct cspt_ctx {
   bool capturing;          // inside cspt_run_cfl's stream capture
   size_t elem;             // sizeof(T)
   // workspace sub-buffers (byte offsets)
-  size_t off_fields, off_inflow, off_scalars;
+  size_t off_fields, off_inflow, off_scalars, off_map;
+  size_t map_bytes;
+  bool map_valid;          // the brick map covers every non-zero cell of the current U^n
+  int tile_skip;           // cspt_debug_tile_skip: 1 (default) = dead CTAs may return early, 0 = never
+  int zero_fill_steps;     // steps in which dead CTAs must still WRITE their zeros: 2 after the map was rebuilt or the
+                           // intermediate slots served as staging (both U buffers and every intermediate get clean)
   long long inflow_plane;  // elements per captured plane
   // TMA views (x, y, z, field) of the two U buffers, of the (U~, xi) group and of the star group
   CUtensorMap mapU[2], mapL, mapS;

@@ -120,7 +120,7 @@ template <class T, int TX, int TY, int LIM, int VAC>
 __global__ void __launch_bounds__(TX* TY, (sizeof(T) == 4 ? 1024 : 512) / (TX * TY))
 k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL, Params<T> P,
                const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, T* __restrict__ UN,
-               typename Real<T>::bits_t* __restrict__ smax_out, int zchunk) {
+               typename Real<T>::bits_t* __restrict__ smax_out, int zchunk, BrickMap M) {
   typedef EulerSmem<T, TX, TY> S;
   extern __shared__ __align__(128) unsigned char sm[];
   uint64_t* bar = (uint64_t*)(sm + S::OFF_BAR);
@@ -134,6 +134,17 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
   const bool inside = i < L.nx && j < L.ny;
   const long long fs = L.fstride;
   constexpr uint32_t TX_BYTES = (uint32_t)((S::U_ELEMS + S::L_ELEMS) * sizeof(T));
+
+  // all of U^n within reach of this CTA exactly 0 (BrickMap): U^{n+1} of its cells is exactly 0, no signal speed
+  if (VAC && M.raw && cta_region_dead(M, L, i0 + GX - 3, i0 + TX + GX + 3, j0 + NG - 3, j0 + TY + NG + 3, z0 + NG - 3, z1 + NG + 3)) {
+    if (inside && M.zero_fill)
+      for (int p = z0; p < z1; ++p) {
+        const long long c = L.idx(i, j, p);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) UN[c + q * fs] = (T)0;
+      }
+    return;
+  }
 
   if (tid == 0) {
     mbar_init(&bar[0], 1);
@@ -314,6 +325,12 @@ k_euler_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
         long long c = L.idx(i, j, p - 1);
 #pragma unroll
         for (int q = 0; q < 5; ++q) UN[c + q * fs] = un[q];
+        if (VAC && M.raw) {                          // the map follows the gas: flag the brick of a non-zero result
+          bool nz = false;
+#pragma unroll
+          for (int q = 0; q < 5; ++q) nz = nz || (un[q] != (T)0);
+          if (nz) brick_flag(M, i + GX, j + NG, p - 1 + NG);
+        }
         // CFL speed of U^{n+1} (G15): exactly rounded, but only for cells whose estimate comes within the
         // filter margin of a speed already known exactly (this thread's maximum or the global one so far);
         // the true maximum always passes the filter, so the result is the exact maximum

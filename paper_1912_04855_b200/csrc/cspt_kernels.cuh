@@ -89,6 +89,49 @@ template <> struct Fast<float> {
   static __device__ __forceinline__ float cancel_eps() { return 9.6e-7f; }
 };
 
+// ---- brick map (cspt_common.cuh, BrickMap) ------------------------------------------------------------------------
+// (px, py, pz): padded coordinates of a cell
+__device__ __forceinline__ void brick_flag(const BrickMap& M, int px, int py, int pz) {
+  M.raw[((size_t)(pz / BRZ) * M.nby + (py / BRY)) * M.nbx + (px / BRX)] = 1;
+}
+// Called by EVERY thread of a 1-D CTA: true if no brick that overlaps the box [x0,x1) x [y0,y1) x [z0,z1) of padded
+// coordinates (clamped to the array) is live.  Flags are only ever added, also while a kernel runs (the Euler stage
+// flags U^{n+1}): a CTA that sees such a flag early merely evaluates zeros in full.
+__device__ __forceinline__ bool cta_region_dead(const BrickMap& M, const Layout& L, int x0, int x1, int y0, int y1, int z0, int z1) {
+  x0 = max(x0, 0); y0 = max(y0, 0); z0 = max(z0, 0);
+  x1 = min(x1, L.px); y1 = min(y1, L.py); z1 = min(z1, L.pz);
+  const int bx0 = x0 / BRX, by0 = y0 / BRY, bz0 = z0 / BRZ;
+  const int ex = (x1 - 1) / BRX - bx0 + 1, ey = (y1 - 1) / BRY - by0 + 1, ez = (z1 - 1) / BRZ - bz0 + 1;
+  int any = 0;
+  if (ex > 0 && ey > 0 && ez > 0) {
+    const int n = ex * ey * ez;
+    for (int t = threadIdx.x; t < n; t += blockDim.x) {
+      const int bx = bx0 + t % ex, r = t / ex, by = by0 + r % ey, bz = bz0 + r / ey;
+      any |= __ldg(M.raw + ((size_t)bz * M.nby + by) * M.nbx + bx);
+    }
+  }
+  const bool dead = !__syncthreads_or(any);
+  if (dead && threadIdx.x == 0) atomicAdd(M.dead, 1ULL);
+  return dead;
+}
+
+// rebuilds the map from the current U over the cells a step can read: interior and the 3 ghost layers
+template <class T>
+__global__ void k_brick_scan(Layout L, const T* __restrict__ U, BrickMap M) {
+  const int ex = L.nx + 2 * NG, ey = L.ny + 2 * NG, ez = L.nz + 2 * NG;
+  const long long n = (long long)ex * ey * ez;
+  for (long long m = blockIdx.x * (long long)blockDim.x + threadIdx.x; m < n; m += (long long)gridDim.x * blockDim.x) {
+    const int i = (int)(m % ex) - NG;
+    const long long r = m / ex;
+    const int j = (int)(r % ey) - NG, k = (int)(r / ey) - NG;
+    const long long c = L.idx(i, j, k);
+    bool nz = false;
+#pragma unroll
+    for (int f = 0; f < 5; ++f) nz = nz || (U[c + f * L.fstride] != (T)0);
+    if (nz) brick_flag(M, i + GX, j + NG, k + NG);
+  }
+}
+
 // ---- set_state: primitives -> conserved, psi into a scratch field ----
 template <class T>
 __global__ void k_set_state(Params<T> P, const T* __restrict__ rho, const T* __restrict__ u,
@@ -161,7 +204,7 @@ __global__ void k_get_state(Params<T> P, const T* __restrict__ U, T* __restrict_
 template <class T>
 __global__ void k_ghost_axis(Layout L, int d, int mode, int bc_lo, int bc_hi, int nfields,
                              T* __restrict__ F, T* __restrict__ inflow_lo, T* __restrict__ inflow_hi,
-                             long long inflow_plane) {
+                             long long inflow_plane, BrickMap M) {
   int n[3] = {L.nx, L.ny, L.nz};
   int d1 = (d + 1) % 3, d2 = (d + 2) % 3;
   int lo1 = d1 < d ? -NG : 0, hi1 = d1 < d ? n[d1] + NG : n[d1];
@@ -185,7 +228,9 @@ __global__ void k_ghost_axis(Layout L, int d, int mode, int bc_lo, int bc_hi, in
     if (kind == CSPT_BC_PERIODIC) {
       s[d] = side ? ((g - 1) % n[d]) : (n[d] - 1 - ((g - 1) % n[d]));
       long long cs = L.idx(s[0], s[1], s[2]);
-      for (int f = 0; f < nfields; ++f) F[cq + f * L.fstride] = F[cs + f * L.fstride];
+      bool nz = false;
+      for (int f = 0; f < nfields; ++f) { T val = F[cs + f * L.fstride]; F[cq + f * L.fstride] = val; nz = nz || (val != (T)0); }
+      if (M.raw && nz) brick_flag(M, q[0] + GX, q[1] + NG, q[2] + NG);
     } else if (mode == 2) {
       s[d] = side ? n[d] - 1 - g : g;
       s[d] = max(0, min(n[d] - 1, s[d]));
@@ -204,6 +249,7 @@ __global__ void k_ghost_axis(Layout L, int d, int mode, int bc_lo, int bc_hi, in
         else val = F[ce + f * L.fstride];
         F[cq + f * L.fstride] = val;
         if (kind == CSPT_BC_INFLOW && mode == 1 && g == 1) inf[f * inflow_plane + pi] = val;
+        if (M.raw && val != (T)0) brick_flag(M, q[0] + GX, q[1] + NG, q[2] + NG);
       }
     }
   }

@@ -84,7 +84,7 @@ template <class T, int TX, int TY, int NSTG = 0>
 __global__ void __launch_bounds__(TX* TY, (sizeof(T) == 4 ? 768 : 512) / (TX * TY))
 k_predictor_stream(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapF, Params<T> P,
                    const DevScalars<T>* __restrict__ sc, const T* __restrict__ U, const T* __restrict__ F,
-                   T* __restrict__ ST, int zchunk, int x0, int x1) {      // particle columns [x0, x1)
+                   T* __restrict__ ST, int zchunk, int x0, int x1, BrickMap M) {      // particle columns [x0, x1)
   typedef PredSmem<T, TX, TY> S;
   typedef PredRing<T, TX, TY, NSTG> R;
   __shared__ T sbuf[2][S::PLANE];
@@ -108,6 +108,28 @@ k_predictor_stream(const __grid_constant__ CUtensorMap mapU, const __grid_consta
   else { int t = tid - 2 * S::BX; hx = (t & 1) ? TX : -1; hy = t >> 1; }
   const int hi = min(i0 + hx, L.nx + 2), hj = min(j0 + hy, L.ny + 2);
   const long long c_own = L.idx(i, j, 0), c_halo = L.idx(hi, hj, 0), sz = L.sz();
+
+  // all inputs within reach of this CTA exactly 0 (BrickMap): the star group of its particles is exactly 0
+  if (M.raw && cta_region_dead(M, L, i0 + GX - 3, i0 + TX + GX + 3, j0 + NG - 3, j0 + TY + NG + 3, z0 + NG - 3, z1 + NG + 3)) {
+    if (valid && M.zero_fill) {
+      typedef typename Pair<T>::type V2;
+      const V2 zero = Pair<T>::make((T)0, (T)0);
+      for (int q = z0; q < z1; ++q) {
+        V2* st2 = (V2*)ST + c_own + (long long)q * sz;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) st2[k * fs] = zero;
+#pragma unroll
+        for (int g = 0; g < 4; ++g) {            // periodic x: the ghost columns this particle wraps onto
+          const int xd = g < 2 ? g - 2 : L.nx + (g - 2);
+          if (x0 == 0 && ((xd % L.nx) + L.nx) % L.nx == i0 + tx) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) st2[xd - (i0 + tx) + k * fs] = zero;
+          }
+        }
+      }
+    }
+    return;
+  }
 
   const T dt = load_dt(sc);
   const T he = (T)0.5 * dt * P.inv_h;
@@ -361,7 +383,7 @@ template <class T, int TX, int TY, int CY, int NST, int MINB, int KERN, int XP>
 __global__ void __launch_bounds__(TX*(TY / CY), MINB)
 k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const DevScalars<T>* __restrict__ sc,
                    const T* __restrict__ U, const T* __restrict__ F, const T* __restrict__ ST, T* __restrict__ UT,
-                   T* __restrict__ XI, int zchunk) {
+                   T* __restrict__ XI, int zchunk, BrickMap M) {
   typedef CorrSmem<T, TX, TY, CY, NST, XP> S;
   typedef Fast<T> FT;
   extern __shared__ __align__(128) unsigned char sm[];
@@ -375,6 +397,36 @@ k_corrector_stream(const __grid_constant__ CUtensorMap mapS, Params<T> P, const 
   const int ly0 = tq * CY;                          // first own row inside the tile
   const long long fs = L.fstride;
   constexpr uint32_t TX_BYTES = (uint32_t)(S::PLANE * sizeof(T));
+
+  // all inputs within reach of this CTA exactly 0 (BrickMap): U~ and xi of its cells are exactly 0
+  if (M.raw && cta_region_dead(M, L, i0 + GX - 3, i0 + TX + GX + 3, j0 + NG - 3, j0 + TY + NG + 3, z0 + NG - 3, z1 + NG + 3)) {
+    for (int p = z0; p < z1 && M.zero_fill; ++p) {
+#pragma unroll
+      for (int c = 0; c < CY; ++c) {
+        const int j = j0 + ly0 + c;
+        if (!(i < L.nx + (XP ? 0 : 1) && j <= L.ny)) continue;
+        const long long cc = L.idx(i, j, p);
+#pragma unroll
+        for (int f = 0; f < 4; ++f) UT[cc + f * fs] = (T)0;
+#pragma unroll
+        for (int f = 0; f < 3; ++f) XI[cc + f * fs] = (T)0;
+        if (XP) {
+#pragma unroll
+          for (int g = 0; g < 2; ++g) {
+            const int xd = g ? L.nx : -1;
+            if (((xd % L.nx) + L.nx) % L.nx == i) {
+              const long long cw = cc + (xd - i);
+#pragma unroll
+              for (int f = 0; f < 4; ++f) UT[cw + f * fs] = (T)0;
+#pragma unroll
+              for (int f = 0; f < 3; ++f) XI[cw + f * fs] = (T)0;
+            }
+          }
+        }
+      }
+    }
+    return;
+  }
 
   if (tid == 0) {
 #pragma unroll
