@@ -570,6 +570,9 @@ def run_cspt(args):
                     "probe": probe, "probe_error": probe_err,
                     "algorithmic_instr_per_cell": ALGO_INSTR[dom], "kernel_ms": dom_ms, "share_of_step": share,
                     "hbm": hbm}
+        if w.name == "disk":
+            roofline["note"] = ("gas-vacuum workload: the instruction list is counted over ALL cells, while CTAs whose "
+                                "inputs are exactly 0 return early (DESIGN.md section 7): not a pipe utilisation here")
     else:
         roofline = dict(hbm, bound="hbm", kernel=dom, traffic=traffic, traffic_source=traffic_src, ncu=ncu_stored, kernel_ms=dom_ms,
                         share_of_step=share)
