@@ -58,8 +58,17 @@ def _worker(rank, world, port, bc, out):
     recv_hi = torch.zeros(n, dtype=torch.float64) if tr.hi is not None else None
     tr.exchange(send_lo if tr.lo is not None else None, send_hi if tr.hi is not None else None, recv_lo, recv_hi)
     dt = tr.min_scalar(torch.tensor([0.5 - 0.1 * rank], dtype=torch.float64))
+    # the signal-speed word of the sync-free protocol: reduced IN PLACE on a view of a larger buffer, in both dtypes
+    ws = torch.zeros(16, dtype=torch.uint8)
+    word = ws[8:16].view(torch.float64)
+    word[0] = 1.0 + 0.25 * rank
+    tr.max_scalar(word)
+    w32 = ws[0:4].view(torch.float32)
+    w32[0] = 3.0 - rank
+    tr.max_scalar(w32)
+    assert not tr.stream_ordered                     # gloo: SlabSolver synchronises before it hands messages over
     out[rank] = (None if recv_lo is None else float(recv_lo[0]), None if recv_hi is None else float(recv_hi[0]),
-                 float(dt[0]))
+                 float(dt[0]), float(ws[8:16].view(torch.float64)[0]), float(ws[0:4].view(torch.float32)[0]))
     dist.barrier()
     dist.destroy_process_group()
 
@@ -73,7 +82,8 @@ def test_transport_delivers_the_right_planes(world, periodic):
         res = dict(out)
     for r in range(world):
         lo, hi = slab.neighbours(bc, r, world)
-        got_lo, got_hi, dt = res[r]
+        got_lo, got_hi, dt, smax64, smax32 = res[r]
+        assert smax64 == 1.0 + 0.25 * (world - 1) and smax32 == 3.0      # maxima over the ranks, in place
         # my lo ghost planes are the HI planes of the rank below, my hi ghost planes the LO planes of the rank above
         assert got_lo == (None if lo is None else 10.0 * lo + 2.0)
         assert got_hi == (None if hi is None else 10.0 * hi + 1.0)
@@ -87,3 +97,4 @@ def test_single_periodic_slab_wraps_without_a_process_group():
     tr.exchange(a, b, rl, rh)
     assert torch.equal(rl, b) and torch.equal(rh, a)
     assert float(tr.min_scalar(torch.tensor([0.25]))[0]) == 0.25
+    assert float(tr.max_scalar(torch.tensor([0.25]))[0]) == 0.25 and not tr.stream_ordered
