@@ -61,6 +61,8 @@ def parse():
                     help="N > 1: independent replicas (default; north_star has no domain decomposition) or ONE grid cut "
                          "into z slabs over the ranks (SURVEY 8(f) NEXT-2, strong scaling)")
     ap.add_argument("--e2e-steps", type=int, default=8)
+    ap.add_argument("--no-tile-skip", action="store_true",
+                    help="fp32 gas-vacuum workloads: switch the CTA-level vacuum shortcut off (cspt_debug_tile_skip(0)), for A/B runs")
     ap.add_argument("--no-configs", action="store_true", help="skip the per-config throughput table")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -416,6 +418,8 @@ def run_cspt(args):
     s = cspt.Solver(w.nx, w.ny, w.nz, w.h, w.gamma, w.bc, dtype)
     if args.kernel == "poly5":
         s.set_kernel(cspt.KERNEL_POLY5)
+    if args.no_tile_skip:
+        s.debug_tile_skip(0)
     s.set_state_host(*fields)
     s.set_limiter(cspt.LIMITER_VANLEER if args.limiter == "vanleer" else cspt.LIMITER_MINMOD)
     s.set_riemann({"hll": cspt.RIEMANN_HLL, "lf": cspt.RIEMANN_LF, "hllc": cspt.RIEMANN_HLLC}[args.riemann])
@@ -585,7 +589,7 @@ def run_cspt(args):
         "ms_per_step": step_ms, "kernels": kern, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": w.dtype, "data": "synthetic",
         "config": dict(config_of(w, world), limiter=args.limiter, kernel=args.kernel, riemann=args.riemann,
-                       api="cspt_run_cfl"),
+                       api="cspt_run_cfl", tile_skip=not args.no_tile_skip),
         "clocks": clocks, "e2e": e2e, "gpu_launches": launches,
         "kernels_note": "per-kernel times from a second pass of the same K steps with an event pair around every launch "
                         "(%.3f ms per step in that pass, %d steps recorded)" % (prof_step_ms, prof_steps),
